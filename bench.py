@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- grid-point updates/s of the relaxation step (fp64, mimetic curl) on BASELINE.json config 4.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4]
+
+One "step" is one pass of the whole hot path (S1-S5: Jacobian, push-forward, mimetic curl, J x B, line-tied
+update) over the full 256x256x512 grid = one fused kernel launch inside mr_step.  The timed region is ONE
+mr_step(K) call bracketed by CUDA events on the launching stream (barrier + synchronize on both sides, max
+over ranks).  Prints ONE JSON line (see DESIGN.md "Measurement" for every key).
+
+Multi-GPU: north_star keeps the path on one GPU ("replicas only"): --gpus N runs N independent
+replicas, one process per GPU (torchrun), value = N * nodes * K / max-over-ranks time, "scaling": "weak".
+
+--impl reference times the CPU oracle (oracle/mro.c) as it stands on the host cores for the same metric, on a
+bounded sample of the same workload.  The oracle is only ever touched by that arm and by the cpu_baseline leg.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "grid-point updates/s (fp64, mimetic curl)"
+UNIT = "updates/s"
+BYTES_PER_UPDATE = {"f64": 72.0, "f32": 36.0}   # read xi 3T + read b 3T + write xi' 3T
+
+
+# ---------------------------------------------------------------------------------------------- helpers (CPU)
+
+def measured_peak_gbs():
+    """HBM roofline denominator: the driver-measured copy bandwidth, else the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def recorded_traffic(workload):
+    """dram bytes per launch from the committed ncu --set full capture (profiles/traffic.json), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(workload, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons every 100 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.rows = []
+        self._stop = threading.Event()
+        self._t = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                for line in out.strip().splitlines():
+                    self.rows.append([c.strip() for c in line.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=10)
+
+    def summary(self):
+        return summarize_clocks(self.rows)
+
+
+def summarize_clocks(rows):
+    sm, mx, reasons = [], [], set()
+    names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+    for r in rows:
+        try:
+            sm.append(float(r[0]))
+            mx.append(float(r[1]))
+        except Exception:
+            continue
+        for name, v in zip(names, r[3:7]):
+            if v.lower().startswith("active"):
+                reasons.add(name)
+    if not sm:
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+    sm.sort()
+    return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def aggregate_over_ranks(local_ms, local_updates, dist=None):
+    """max-over-ranks time and summed work (torch.distributed when world_size > 1)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_ms, local_updates
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([local_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([float(local_updates)], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def workload(name):
+    from paper_1405_0942_b200 import inputs as I
+    cfg = I.CONFIGS[name]
+    return cfg, I
+
+
+# ---------------------------------------------------------------------------------------------- oracle legs
+
+def oracle_sample(cfg, I, budget_s=12.0, planes=64):
+    """Time the CPU oracle, as it stands, on a bounded sample of the workload: the first `planes` z-planes of the
+    grid (same spacing and field) for as many steps as fit the budget.  Returns (updates/s, threads, description)."""
+    import numpy as np
+    from oracle import mro                       # the ONLY place bench.py touches the oracle
+    g = cfg.grid
+    nz = min(planes, g.n[2])
+    sub = I.Grid((g.n[0], g.n[1], nz), g.lo, (g.hi[0], g.hi[1], g.lo[2] + (nz - 1) * g.h[2]))
+    B0 = I.twist_field(sub, cfg.twists) if cfg.twists else I.abc_field(I.reference_grid(sub))
+    x0 = I.reference_grid(sub)
+    dt = I.stable_dt(B0, sub)
+    threads = mro.max_threads()
+    mro.set_threads(threads)
+    t0 = time.perf_counter()
+    x = mro.step(sub.n, sub.lo, sub.hi, x0, B0, dt, 1)
+    t1 = time.perf_counter() - t0
+    steps = int(max(1, min(20, budget_s / max(t1, 1e-3))))
+    t0 = time.perf_counter()
+    mro.step(sub.n, sub.lo, sub.hi, x, B0, dt, steps)
+    el = time.perf_counter() - t0
+    mro.set_threads(1)
+    desc = "%s z-slab %dx%dx%d (same h and B0), %d Euler steps, mimetic, OpenMP over k" % (cfg.name, sub.n[0], sub.n[1], sub.n[2], steps)
+    return sub.nodes * steps / el, threads, desc
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/config; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg, I = workload(args.workload)
+    import numpy as np
+    from oracle import mro
+    g = cfg.grid
+    planes = 16
+    sub = I.Grid((g.n[0], g.n[1], planes), g.lo, (g.hi[0], g.hi[1], g.lo[2] + (planes - 1) * g.h[2]))
+    B0 = I.twist_field(sub, cfg.twists)
+    x = I.reference_grid(sub)
+    dt = I.stable_dt(B0, sub)
+    threads = mro.max_threads()
+    mro.set_threads(threads)
+    for _ in range(args.warmup):
+        x = mro.step(sub.n, sub.lo, sub.hi, x, B0, dt, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        x = mro.step(sub.n, sub.lo, sub.hi, x, B0, dt, 1)
+    el = time.perf_counter() - t0
+    value = sub.nodes * args.steps / el
+    sample = "%s z-slab %dx%dx%d per step (same h and B0), mimetic, OpenMP over k" % (cfg.name, sub.n[0], sub.n[1], sub.n[2])
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s %dx%dx%d fp64 mimetic (CPU oracle on a z-slab sample)" % ((cfg.name,) + g.n)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------- our arm (GPU)
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the relaxation step has no CPU path")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_1405_0942_b200 import mr   # fails loudly if libmr.so is missing
+
+    cfg, I = workload(args.workload)
+    g = cfg.grid
+    dtype = cfg.dtype
+    td = torch.float64 if dtype == "f64" else torch.float32
+    x0, B0, dt = I.make(cfg)
+    nodes = g.nodes
+
+    sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype, device="cuda:%d" % local_rank)
+    if args.variant != "auto":
+        sim.set_variant(args.variant)
+    B0_d = torch.from_numpy(B0).to("cuda", dtype=td)
+    x0_d = torch.from_numpy(x0).to("cuda", dtype=td)
+    sim.set_B0(B0_d)
+    sim.set_x(x0_d)
+    del B0_d
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-up steps, then ONE timed mr_step(K) ----
+    sim.step(max(args.warmup, 3), dt)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local_rank) as clocks:
+        l0 = sim.launch_count
+        e0.record()
+        sim.step(args.steps, dt)
+        e1.record()
+        barrier()
+        launches = sim.launch_count - l0
+    ms = e0.elapsed_time(e1)
+    variant = sim.step_variant
+    ms_all, updates_all = aggregate_over_ranks(ms, nodes * args.steps, dist if world > 1 else None)
+    value = updates_all / (ms_all * 1e-3)
+    diag = sim.diagnostics()
+
+    # ---- roofline of the dominant (only) kernel: algorithmic bytes per launch / average launch duration ----
+    peak, peak_src = measured_peak_gbs()
+    launch_ms = ms / max(launches, 1)
+    achieved = BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": recorded_traffic(cfg.name), "peak_source": peak_src, "kernel": variant,
+                "algorithmic_bytes_per_launch": BYTES_PER_UPDATE[dtype] * nodes, "launch_ms": launch_ms}
+
+    # ---- end to end through the host-buffer entry points: H2D of x, one step, D2H of x, every step ----
+    xh = torch.from_numpy(x0).to(td).pin_memory()
+    oh = torch.empty_like(xh).pin_memory()
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    sim.set_x(xh)
+    sim.step(1, dt)
+    sim.get_fields_into(x=oh)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sim.set_x(xh)                 # mr_set_x_host: pinned host -> device (+ layout import)
+        sim.step(1, dt)               # mr_step
+        sim.get_fields_into(x=oh)     # mr_get_fields_host: device -> pinned host
+        xh, oh = oh, xh
+    barrier()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    e2e_ms_all, e2e_updates = aggregate_over_ranks(e2e_ms, nodes * e2e_steps, dist if world > 1 else None)
+    fbytes = 3 * nodes * (8 if dtype == "f64" else 4)
+    e2e = {"value": e2e_updates / (e2e_ms_all * 1e-3), "unit": UNIT, "h2d_bytes_per_step": fbytes,
+           "d2h_bytes_per_step": fbytes, "steps": e2e_steps,
+           "what": "per step: mr_set_x_host (pinned H2D of x) + mr_step(1) + mr_get_fields_host (D2H of x)"}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, threads, desc = oracle_sample(cfg, I)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": dtype, "data": "synthetic",
+            "config": {"workload": "%s %dx%dx%d %s mimetic, line-tied, forward Euler dt=%.3e" % ((cfg.name,) + g.n + ("fp64" if dtype == "f64" else "fp32", dt)),
+                       "nodes": nodes, "l2_policy": "working set %.2f GB >> 126 MB L2 (no flush needed)" % (3 * fbytes / 1e9),
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "kernel": variant},
+            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+            "state_after": {"steps": diag["steps"], "energy": diag["energy"], "max_jxb": diag["max_jxb"], "xi": diag["xi"],
+                            "min_det": diag["min_det"]},
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "stream"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,137 @@
+/*
+ * mr.h -- C-ABI boundary of the B200-native Lagrangian magneto-frictional relaxation step
+ * (Candelaresi, Pontin & Hornig, arxiv 1405.0942; citations are PAPER.md line numbers).
+ *
+ * The library advances the Lagrangian map x(X,t) of a structured 3-D grid under u = gamma J x B (Eq. 1.5,
+ * PAPER.md:40) with the frozen-in field B = (dx/dX) B(X,0) / det(dx/dX) (Eq. 2.1, :59), J = curl B by the
+ * nearest-neighbour mimetic operator (Eqs. 2.2-2.7, :68-105) or by the direct-derivative ("classical") variant
+ * (:49, :257), line-tied boundaries (:147), and the grid-wide diagnostics E_M (Eq. 3.13, :251) and
+ * xi = max |J x B|/B^2 (Eq. 4.1, :264).  Every step of that path runs in hand-written sm_100a CUDA kernels;
+ * there is no CPU fallback.
+ *
+ * Conventions
+ *   - A vector field on the grid is a dense array T[3][nz][ny][nx] (component-major, i fastest:
+ *     idx = (k*ny + j)*nx + i), T = double (MR_F64) or float (MR_F32).
+ *   - Reference grid X_ijk = lo + idx*h, h_a = (hi_a - lo_a)/(n_a - 1); nodes include the boundary (:170).
+ *   - "_dev" pointers are CUDA device pointers on the context's device; "_host" pointers are host pointers
+ *     (pinned memory makes the copies asynchronous and fast, pageable memory also works).
+ *   - Ownership: the CALLER owns every device and host buffer and the stream.  The library never allocates
+ *     device memory: mr_create binds a caller-provided workspace of at least mr_workspace_bytes() bytes
+ *     (256-byte aligned) that must outlive the context.  mr_ctx itself is host memory owned by the library.
+ *   - All work is enqueued on the caller's stream.  mr_step, mr_diagnostics and the *_host calls synchronise
+ *     that stream before returning; mr_set_B0, mr_set_x and mr_get_fields are asynchronous.
+ *   - Errors are return codes; nothing throws or aborts.  mr_last_error(ctx) gives a message for the last
+ *     failing call on that context.  After MR_ERR_NUMERIC the context stays failed until mr_set_x succeeds.
+ */
+#ifndef MR_H_
+#define MR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mr_ctx mr_ctx; /* opaque */
+
+typedef enum {
+    MR_OK = 0,
+    MR_ERR_INVALID_ARG = 1, /* null pointer, bad size, unsupported option */
+    MR_ERR_WORKSPACE = 2,   /* workspace null, misaligned or too small */
+    MR_ERR_CUDA = 3,        /* a CUDA runtime/driver call failed (no device, launch failure, ...) */
+    MR_ERR_STATE = 4,       /* B0 has not been set */
+    MR_ERR_NUMERIC = 5      /* det(dx/dX) <= 0 or a non-finite value was met (grid folded, cf. :333) */
+} mr_status;
+
+typedef enum {
+    MR_OP_MIMETIC = 0, /* Eqs. 2.3-2.7 (:68-105): three Stokes loops through the 4 nearest neighbours */
+    MR_OP_DIRECT = 1   /* analytic derivative of Eq. 2.1: products of 1st and 2nd differences of x (:49) */
+} mr_operator;
+
+typedef enum {
+    MR_BC_LINE_TIED = 0, /* u = 0 and B.n fixed on the face (:147) */
+    MR_BC_PERIODIC = 1   /* Eqs. 2.12-2.14; NOT IMPLEMENTED: mr_create returns MR_ERR_INVALID_ARG */
+} mr_bc;
+
+typedef enum { MR_F64 = 0, MR_F32 = 1 } mr_dtype;
+
+typedef struct { int32_t nx, ny, nz; } mr_grid;      /* nodes per logical axis, each 5 <= n <= 4096 */
+typedef struct { double lo[3], hi[3]; } mr_domain;   /* hi > lo componentwise */
+
+/* "boundary" + options of mr_create */
+typedef struct {
+    mr_bc bc[3];            /* per logical axis (both faces); only MR_BC_LINE_TIED is implemented */
+    double gamma;           /* > 0; Eq. 1.5, the paper uses 1 (:55) */
+    mr_dtype dtype;         /* storage and arithmetic type of the state; reductions always accumulate in fp64 */
+    void* workspace;        /* device pointer, >= mr_workspace_bytes(), 256-byte aligned, caller-owned */
+    size_t workspace_bytes;
+    void* stream;           /* cudaStream_t (0 = legacy default stream), caller-owned */
+} mr_boundary;
+
+typedef struct {
+    double time;     /* sum of dt over all steps taken since the last mr_set_x / mr_create */
+    int64_t steps;   /* number of steps taken since then */
+    double energy;   /* E_M = 1/2 sum zeta |B|^2 Delta dXdYdZ over all nodes, zeta = 1/2 per face (Eq. 3.13) */
+    double max_jxb;  /* max over interior nodes of |J x B| */
+    double xi;       /* max over interior nodes of |J x B| / |B|^2 (Eq. 4.1) */
+    double min_det;  /* min over all nodes of Delta = det(dx/dX) */
+} mr_diag;
+
+/* Bytes of device workspace mr_create needs for this grid and dtype (0 if the arguments are invalid).
+ * Holds the double-buffered state, the pre-scaled B(X,0), a staging buffer for the *_host calls and the
+ * reduction partials; about 4 fields = 12*nx*ny*nz elements.  Pure host arithmetic, needs no GPU. */
+size_t mr_workspace_bytes(const mr_grid* grid, mr_dtype dtype);
+
+/* Create a context on the current CUDA device; the state is initialised to x = X.
+ * Returns MR_ERR_INVALID_ARG for bad sizes/options (checked before any CUDA call), MR_ERR_WORKSPACE,
+ * MR_ERR_CUDA (e.g. no sm_100 device).  On failure *out is NULL. */
+mr_status mr_create(const mr_grid* grid, const mr_domain* domain, const mr_boundary* boundary, mr_ctx** out);
+
+/* Free the host-side context (the workspace stays with the caller).  NULL is allowed. */
+mr_status mr_destroy(mr_ctx* ctx);
+
+/* Set the initial field B(X,0) at the nodes (Eq. 2.1): dense T[3][nz][ny][nx] in the context dtype; copied
+ * (and pre-scaled) into the workspace, the source may be reused once the stream has passed this call. */
+mr_status mr_set_B0(mr_ctx* ctx, const void* B0_dev);
+mr_status mr_set_B0_host(mr_ctx* ctx, const void* B0_host);
+
+/* Set the node positions x (dense, context dtype), e.g. a displaced initial grid or a checkpoint; resets
+ * time/steps and clears a numeric failure.  Line-tied boundary nodes must equal X (|x - X| <= 1e-6*h),
+ * otherwise MR_ERR_INVALID_ARG is returned and the state is unchanged.  (Synchronises for that check.) */
+mr_status mr_set_x(mr_ctx* ctx, const void* x_dev);
+mr_status mr_set_x_host(mr_ctx* ctx, const void* x_host);
+
+/* Take n >= 0 explicit steps x <- x + dt * gamma * J x B on interior nodes, boundary nodes fixed (Eq. 1.2,
+ * :17; :147), all velocities from the old x.  dt > 0.  Synchronises the stream at the end and returns
+ * MR_ERR_NUMERIC if any node had det <= 0 or a non-finite value during these steps, MR_ERR_STATE without B0. */
+mr_status mr_step(mr_ctx* ctx, int64_t n, double dt, mr_operator op);
+
+/* Grid-wide reduction of the CURRENT state (no update): fills *out.  Deterministic (fixed-order two-stage
+ * reduction).  Synchronises the stream. */
+mr_status mr_diagnostics(mr_ctx* ctx, mr_operator op, mr_diag* out);
+
+/* Materialise fields of the current state into caller buffers (dense, context dtype); any pointer may be
+ * NULL.  x = node positions; B = pushed-forward field on ALL nodes; J = current on interior nodes by `op`,
+ * 0 on boundary nodes. */
+mr_status mr_get_fields(mr_ctx* ctx, mr_operator op, void* x_dev, void* B_dev, void* J_dev);
+mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_host, void* B_host, void* J_host);
+
+/* Message for the last error on this context ("" if none); ctx == NULL gives the last mr_create failure.
+ * The pointer stays valid until the next failing call on the same context (or mr_destroy). */
+const char* mr_last_error(const mr_ctx* ctx);
+
+/* Introspection for benchmarks and tests: number of kernel launches issued by this context so far, and the
+ * name of the step-kernel variant the last mr_step used ("" before the first step). */
+int64_t mr_launch_count(const mr_ctx* ctx);
+const char* mr_step_variant(const mr_ctx* ctx);
+
+/* Choose the step kernel: "auto" (default: the streaming TMA kernel when it takes the grid and operator, else
+ * the generic one), "generic" (always the global-memory kernel; the A/B reference), "stream" (mr_step fails
+ * with MR_ERR_INVALID_ARG if the streaming kernel cannot be used).  Results agree to rounding. */
+mr_status mr_set_variant(mr_ctx* ctx, const char* name);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MR_H_ */

@@ -1,0 +1,226 @@
+"""Thin ctypes binding of the C-ABI library ``libmr.so`` (include/mr.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels.  PyTorch supplies device memory (the
+workspace and the field tensors) and the CUDA stream; nothing here computes.  Importing this module fails loudly
+if ``libmr.so`` has not been built (``python -m paper_1405_0942_b200.build``); there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmr.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        "paper_1405_0942_b200: %s is missing -- build it with `python -m paper_1405_0942_b200.build` "
+        "(nvcc, sm_100a).  There is no CPU fallback for the relaxation step." % LIB_PATH)
+
+lib = C.CDLL(LIB_PATH)
+
+# ---- enums (include/mr.h) ---------------------------------------------------------------------------------
+MR_OK, MR_ERR_INVALID_ARG, MR_ERR_WORKSPACE, MR_ERR_CUDA, MR_ERR_STATE, MR_ERR_NUMERIC = range(6)
+MR_OP_MIMETIC, MR_OP_DIRECT = 0, 1
+MR_BC_LINE_TIED, MR_BC_PERIODIC = 0, 1
+MR_F64, MR_F32 = 0, 1
+
+STATUS_NAMES = {0: "MR_OK", 1: "MR_ERR_INVALID_ARG", 2: "MR_ERR_WORKSPACE", 3: "MR_ERR_CUDA", 4: "MR_ERR_STATE",
+                5: "MR_ERR_NUMERIC"}
+OPERATORS = {"mimetic": MR_OP_MIMETIC, "direct": MR_OP_DIRECT}
+
+
+class mr_grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32)]
+
+
+class mr_domain(C.Structure):
+    _fields_ = [("lo", C.c_double * 3), ("hi", C.c_double * 3)]
+
+
+class mr_boundary(C.Structure):
+    _fields_ = [("bc", C.c_int * 3), ("gamma", C.c_double), ("dtype", C.c_int), ("workspace", C.c_void_p),
+                ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p)]
+
+
+class mr_diag(C.Structure):
+    _fields_ = [("time", C.c_double), ("steps", C.c_int64), ("energy", C.c_double), ("max_jxb", C.c_double),
+                ("xi", C.c_double), ("min_det", C.c_double)]
+
+
+_ctx_p = C.c_void_p
+lib.mr_workspace_bytes.argtypes = [C.POINTER(mr_grid), C.c_int]
+lib.mr_workspace_bytes.restype = C.c_size_t
+lib.mr_create.argtypes = [C.POINTER(mr_grid), C.POINTER(mr_domain), C.POINTER(mr_boundary), C.POINTER(_ctx_p)]
+lib.mr_create.restype = C.c_int
+lib.mr_destroy.argtypes = [_ctx_p]
+lib.mr_destroy.restype = C.c_int
+for _n in ("mr_set_B0", "mr_set_B0_host", "mr_set_x", "mr_set_x_host"):
+    getattr(lib, _n).argtypes = [_ctx_p, C.c_void_p]
+    getattr(lib, _n).restype = C.c_int
+lib.mr_step.argtypes = [_ctx_p, C.c_int64, C.c_double, C.c_int]
+lib.mr_step.restype = C.c_int
+lib.mr_diagnostics.argtypes = [_ctx_p, C.c_int, C.POINTER(mr_diag)]
+lib.mr_diagnostics.restype = C.c_int
+for _n in ("mr_get_fields", "mr_get_fields_host"):
+    getattr(lib, _n).argtypes = [_ctx_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+    getattr(lib, _n).restype = C.c_int
+lib.mr_last_error.argtypes = [_ctx_p]
+lib.mr_last_error.restype = C.c_char_p
+lib.mr_launch_count.argtypes = [_ctx_p]
+lib.mr_launch_count.restype = C.c_int64
+lib.mr_step_variant.argtypes = [_ctx_p]
+lib.mr_step_variant.restype = C.c_char_p
+lib.mr_set_variant.argtypes = [_ctx_p, C.c_char_p]
+lib.mr_set_variant.restype = C.c_int
+
+
+class MrError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (STATUS_NAMES.get(status, status), message))
+        self.status = status
+
+
+class NumericError(MrError):
+    """MR_ERR_NUMERIC: det(dx/dX) <= 0 or a non-finite value (the grid folded)."""
+
+
+def _raise(status, ctx):
+    msg = (lib.mr_last_error(ctx) or b"").decode()
+    raise (NumericError if status == MR_ERR_NUMERIC else MrError)(status, msg)
+
+
+def workspace_bytes(n, dtype="f64") -> int:
+    g = mr_grid(*[int(v) for v in n])
+    return int(lib.mr_workspace_bytes(C.byref(g), MR_F64 if dtype == "f64" else MR_F32))
+
+
+def _op(op):
+    return OPERATORS[op] if isinstance(op, str) else int(op)
+
+
+class Relaxation:
+    """mr_create / mr_set_B0 / mr_set_x / mr_step / mr_diagnostics / mr_get_fields on one CUDA device.
+
+    ``n=(nx,ny,nz)``, ``lo``/``hi`` the domain corners; ``dtype`` "f64" or "f32"; fields are torch CUDA tensors
+    (or pinned/pageable host tensors for the ``*_host`` calls) of shape ``(3, nz, ny, nx)`` in that dtype.
+    """
+
+    def __init__(self, n, lo, hi, dtype="f64", gamma=1.0, bc=("line_tied",) * 3, device="cuda", stream=None):
+        import torch
+
+        self._torch = torch
+        self.n = tuple(int(v) for v in n)
+        self.shape = (3, self.n[2], self.n[1], self.n[0])
+        self.dtype = dtype
+        self.tdtype = torch.float64 if dtype == "f64" else torch.float32
+        self.device = torch.device(device)
+        if self.device.type != "cuda":
+            raise MrError(MR_ERR_INVALID_ARG, "the relaxation step runs on a CUDA device only")
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
+        self._ctx = _ctx_p()
+        nbytes = workspace_bytes(self.n, dtype)
+        if nbytes == 0:
+            raise MrError(MR_ERR_INVALID_ARG, "invalid grid %r / dtype %r" % (self.n, dtype))
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            g = mr_grid(*self.n)
+            d = mr_domain((C.c_double * 3)(*[float(v) for v in lo]), (C.c_double * 3)(*[float(v) for v in hi]))
+            bcs = (C.c_int * 3)(*[MR_BC_LINE_TIED if b == "line_tied" else MR_BC_PERIODIC for b in bc])
+            b = mr_boundary(bcs, float(gamma), MR_F64 if dtype == "f64" else MR_F32, self.workspace.data_ptr(),
+                            nbytes, self.stream.cuda_stream)
+            st = lib.mr_create(C.byref(g), C.byref(d), C.byref(b), C.byref(self._ctx))
+        if st != MR_OK:
+            self._ctx = _ctx_p()
+            _raise(st, None)
+
+    # -- helpers ----------------------------------------------------------------------------------------
+    def _check(self, st):
+        if st != MR_OK:
+            _raise(st, self._ctx)
+
+    def _dev(self, t, name):
+        if t is None:
+            return None
+        if t.device != self.device or t.dtype != self.tdtype or tuple(t.shape) != self.shape or not t.is_contiguous():
+            raise MrError(MR_ERR_INVALID_ARG, "%s must be a contiguous %s tensor of shape %r on %s"
+                          % (name, self.tdtype, self.shape, self.device))
+        return t.data_ptr()
+
+    def _host(self, t, name):
+        if t is None:
+            return None
+        if t.device.type != "cpu" or t.dtype != self.tdtype or tuple(t.shape) != self.shape or not t.is_contiguous():
+            raise MrError(MR_ERR_INVALID_ARG, "%s must be a contiguous CPU %s tensor of shape %r" % (name, self.tdtype, self.shape))
+        return t.data_ptr()
+
+    def empty_field(self):
+        return self._torch.empty(self.shape, dtype=self.tdtype, device=self.device)
+
+    # -- the C-ABI calls ----------------------------------------------------------------------------------
+    def set_B0(self, B0):
+        with self._torch.cuda.device(self.device):
+            if B0.device.type == "cpu":
+                self._check(lib.mr_set_B0_host(self._ctx, self._host(B0, "B0")))
+            else:
+                self._check(lib.mr_set_B0(self._ctx, self._dev(B0, "B0")))
+
+    def set_x(self, x):
+        with self._torch.cuda.device(self.device):
+            if x.device.type == "cpu":
+                self._check(lib.mr_set_x_host(self._ctx, self._host(x, "x")))
+            else:
+                self._check(lib.mr_set_x(self._ctx, self._dev(x, "x")))
+
+    def step(self, n, dt, op="mimetic"):
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_step(self._ctx, int(n), float(dt), _op(op)))
+
+    def diagnostics(self, op="mimetic"):
+        out = mr_diag()
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_diagnostics(self._ctx, _op(op), C.byref(out)))
+        return {"time": out.time, "steps": out.steps, "energy": out.energy, "max_jxb": out.max_jxb, "xi": out.xi,
+                "min_det": out.min_det}
+
+    def get_fields(self, op="mimetic", x=False, B=False, J=False, host=False):
+        """Returns the requested fields as new tensors (device, or pinned host with ``host=True``) in a dict."""
+        torch = self._torch
+        out = {}
+        for name, want in (("x", x), ("B", B), ("J", J)):
+            if want:
+                out[name] = (torch.empty(self.shape, dtype=self.tdtype, pin_memory=True) if host else self.empty_field())
+        self.get_fields_into(op, out.get("x"), out.get("B"), out.get("J"))
+        return out
+
+    def get_fields_into(self, op="mimetic", x=None, B=None, J=None):
+        host = any(t is not None and t.device.type == "cpu" for t in (x, B, J))
+        with self._torch.cuda.device(self.device):
+            if host:
+                self._check(lib.mr_get_fields_host(self._ctx, _op(op), self._host(x, "x"), self._host(B, "B"), self._host(J, "J")))
+            else:
+                self._check(lib.mr_get_fields(self._ctx, _op(op), self._dev(x, "x"), self._dev(B, "B"), self._dev(J, "J")))
+
+    def set_variant(self, name):
+        self._check(lib.mr_set_variant(self._ctx, name.encode()))
+
+    @property
+    def launch_count(self):
+        return int(lib.mr_launch_count(self._ctx))
+
+    @property
+    def step_variant(self):
+        return (lib.mr_step_variant(self._ctx) or b"").decode()
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            lib.mr_destroy(self._ctx)
+            self._ctx = _ctx_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,303 @@
+"""GPU parity tests proper: the CUDA path (through the C-ABI, via the ctypes binding) against the CPU oracle on the
+same seeded inputs.  Tolerances (north_star / DESIGN.md Q19): norm-wise relative error per field
+max|a-b| / max|b|  <= 1e-12 after one step, <= 1e-9 after 100 steps (fp64); fp32 variant <= 1e-5.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import mro  # noqa: E402  (test infrastructure)
+from paper_1405_0942_b200 import inputs as I  # noqa: E402
+
+TOL_STEP = 1e-12
+TOL_100 = 1e-9
+TOL_F32 = 1e-5
+
+
+@pytest.fixture(scope="module")
+def mr():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1405_0942_b200 import mr as m
+    return m
+
+
+@pytest.fixture(scope="module", autouse=True)
+def oracle_threads():
+    mro.set_threads(mro.max_threads())
+    yield
+    mro.set_threads(1)
+
+
+def nrel(a, b):
+    """norm-wise relative error of a field (Q19)"""
+    return float(np.abs(np.asarray(a) - np.asarray(b)).max() / max(np.abs(b).max(), 1e-300))
+
+
+def dev(a, dtype=torch.float64):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda", dtype=dtype)
+
+
+def make_sim(mr, g, x0, B0, dtype="f64", variant=None):
+    td = torch.float64 if dtype == "f64" else torch.float32
+    sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype)
+    if variant:
+        sim.set_variant(variant)
+    sim.set_B0(dev(B0, td))
+    sim.set_x(dev(x0, td))
+    return sim
+
+
+def fields_np(sim, op):
+    f = sim.get_fields(op, x=True, B=True, J=True)
+    return {k: v.double().cpu().numpy() for k, v in f.items()}
+
+
+def case(name):
+    """(grid, x0, B0, dt) for the parity cases: sizes the oracle finishes in seconds that still span several
+    tiles with a ragged tail."""
+    if name == "C1":
+        cfg = I.CONFIGS["C1"]
+        x0, B0, dt = I.make(cfg)
+        return cfg.grid, x0, B0, dt
+    if name == "C1_rough":      # C1 field on a non-smoothly distorted grid
+        cfg = I.CONFIGS["C1"]
+        _, B0, dt = I.make(cfg)
+        return cfg.grid, I.rough_displacement(cfg.grid, 0.2, seed=5), B0, dt
+    if name == "ragged":        # odd sizes: row padding, partial tiles in every direction
+        g = I.Grid((37, 21, 13), (-4.0, -4.0, -8.0), (4.0, 4.0, 8.0))
+        B0 = I.twist_field(g, (I.Twist(1.0, 0.3, -0.2, 0.4), I.Twist(-0.7, -1.0, 0.5, -3.0)))
+        return g, I.displaced_grid(g, 0.3, seed=7), B0, 0.5 * I.stable_dt(B0, g)
+    if name == "minimal":       # the smallest legal grid
+        g = I.Grid((5, 5, 5), (-1.0, -1.0, -1.0), (1.0, 1.0, 1.0))
+        B0 = I.twist_field(g, (I.Twist(0.5, 0.0, 0.0, 0.0, a=1.0, l=1.0),))
+        return g, I.displaced_grid(g, 0.2, seed=3), B0, 0.25 * I.stable_dt(B0, g)
+    if name == "wide":          # several tiles in x and y, few planes
+        g = I.Grid((130, 70, 9), (-4.0, -4.0, -2.0), (4.0, 4.0, 2.0))
+        B0 = I.twist_field(g, (I.Twist(1.0, 1.0, 0.0, 0.0), I.Twist(-1.0, -1.0, 0.0, 0.5)))
+        return g, I.displaced_grid(g, 0.3, seed=9), B0, 0.5 * I.stable_dt(B0, g)
+    if name == "C2_small":      # config 2 field at a quarter of the resolution
+        cfg = I.scaled(I.CONFIGS["C2"], (32, 32, 96))
+        x0, B0, dt = I.make(cfg)
+        return cfg.grid, x0, B0, dt
+    if name == "C3_small":      # config 3 (reading D) at 48^3
+        cfg = I.scaled(I.CONFIGS["C3"], (48, 48, 48))
+        x0, B0, dt = I.make(cfg)
+        return cfg.grid, x0, B0, dt
+    raise KeyError(name)
+
+
+CASES = ["C1", "C1_rough", "ragged", "minimal", "wide", "C2_small", "C3_small"]
+
+
+@pytest.mark.parametrize("name", CASES)
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_fields_match_oracle(mr, name, op):
+    """S1-S3: B on all nodes, J on interior nodes (0 on the boundary), x round trip."""
+    g, x0, B0, dt = case(name)
+    sim = make_sim(mr, g, x0, B0)
+    f = fields_np(sim, op)
+    B, J, u, det = mro.fields(g.n, g.lo, g.hi, x0, B0, op=mro.MIMETIC if op == "mimetic" else mro.DIRECT)
+    assert nrel(f["x"], x0) < 1e-15
+    assert nrel(f["B"], B) < TOL_STEP
+    assert nrel(f["J"], J) < TOL_STEP
+    Jb = f["J"].copy()
+    Jb[:, 1:-1, 1:-1, 1:-1] = 0
+    assert np.abs(Jb).max() == 0.0
+
+
+@pytest.mark.parametrize("name", CASES)
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+@pytest.mark.parametrize("variant", ["auto", "generic"])
+def test_one_step_matches_oracle(mr, name, op, variant):
+    """S1-S5 fused: x after one step, also measured on the displacement moved in that step."""
+    g, x0, B0, dt = case(name)
+    sim = make_sim(mr, g, x0, B0, variant=variant)
+    sim.step(1, dt, op)
+    x1 = sim.get_fields(op, x=True)["x"].cpu().numpy()
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 1, op=mro.MIMETIC if op == "mimetic" else mro.DIRECT)
+    assert nrel(x1, ref) < TOL_STEP
+    moved = np.abs(ref - x0).max()
+    assert moved > 0
+    assert np.abs(x1 - ref).max() < 1e-10 * moved + 1e-15 * np.abs(ref).max()
+    # line-tied: boundary nodes did not move at all
+    m = np.ones(x1.shape, bool)
+    m[:, 1:-1, 1:-1, 1:-1] = False
+    assert np.array_equal(x1[m], np.asarray(x0)[m])
+
+
+@pytest.mark.parametrize("name,steps", [("C1", 100), ("C2_small", 100), ("C3_small", 100), ("ragged", 100)])
+@pytest.mark.parametrize("variant", ["auto", "generic"])
+def test_100_steps_match_oracle(mr, name, steps, variant):
+    g, x0, B0, dt = case(name)
+    sim = make_sim(mr, g, x0, B0, variant=variant)
+    sim.step(steps, dt, "mimetic")
+    x = sim.get_fields(x=True)["x"].cpu().numpy()
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, steps)
+    assert nrel(x, ref) < TOL_100
+    assert nrel(x - x0, ref - x0) < 1e-7       # on the displacement itself
+    d = sim.diagnostics("mimetic")
+    assert d["steps"] == steps and d["time"] == pytest.approx(steps * dt, rel=1e-12)
+    o = mro.diagnostics(g.n, g.lo, g.hi, ref, B0)
+    for k in ("energy", "max_jxb", "xi", "min_det"):
+        assert d[k] == pytest.approx(o[k], rel=1e-8)
+
+
+def test_100_direct_steps_match_oracle(mr):
+    g, x0, B0, dt = case("C1")
+    sim = make_sim(mr, g, x0, B0)
+    sim.step(100, dt, "direct")
+    x = sim.get_fields(x=True)["x"].cpu().numpy()
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 100, op=mro.DIRECT)
+    assert nrel(x, ref) < TOL_100
+
+
+@pytest.mark.parametrize("name", CASES)
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_diagnostics_match_oracle(mr, name, op):
+    """S6: energy, max|JxB|, xi, min det within 1e-12 relative; deterministic (bitwise repeatable)."""
+    g, x0, B0, dt = case(name)
+    sim = make_sim(mr, g, x0, B0)
+    d = sim.diagnostics(op)
+    o = mro.diagnostics(g.n, g.lo, g.hi, x0, B0, op=mro.MIMETIC if op == "mimetic" else mro.DIRECT)
+    for k in ("energy", "max_jxb", "xi", "min_det"):
+        assert d[k] == pytest.approx(o[k], rel=TOL_STEP), k
+    assert sim.diagnostics(op) == d
+
+
+def test_config3_reading_P_curl_errors(mr):
+    """Config 3, reading P (B0 pulled back so that the nodal pushed-forward field is ABC(x0)): both curl errors are
+    the oracle's, the mimetic one is the smaller, and the field stays near force-free over 50 steps."""
+    cfg = I.scaled(I.CONFIGS["C3"], (48, 48, 48))
+    g = cfg.grid
+    x0 = I.displaced_grid(g, 0.3)
+    F, det = mro.jacobian(g.n, g.lo, g.hi, x0)
+    Fi = np.linalg.inv(np.moveaxis(F, (0, 1), (-2, -1)))
+    B0 = np.ascontiguousarray(np.einsum("...ac,c...->a...", Fi, I.abc_field(x0)) * det)
+    dt = I.stable_dt(B0, g)
+    sim = make_sim(mr, g, x0, B0)
+    errs = {}
+    for op, code in (("mimetic", 0), ("direct", 1)):
+        f = fields_np(sim, op)
+        _, J, _, _ = mro.fields(g.n, g.lo, g.hi, x0, B0, op=code)
+        assert nrel(f["B"], I.abc_field(x0)) < 1e-12
+        assert nrel(f["J"], J) < TOL_STEP
+        inner = (slice(None), slice(1, -1), slice(1, -1), slice(1, -1))
+        errs[op] = np.abs(f["J"][inner] - np.pi * f["B"][inner]).max() / (np.pi * np.abs(f["B"]).max())
+    assert errs["mimetic"] < errs["direct"] < 0.02
+    f0 = sim.diagnostics()["max_jxb"]
+    sim.step(50, dt)
+    assert sim.diagnostics()["max_jxb"] < 2.0 * f0 + 1e-3      # stays (near) force-free
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 50)
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), ref) < TOL_100
+
+
+def test_abc_on_undistorted_grid_does_not_move(mr):
+    g = I.Grid((32, 32, 32), (-1.0, -1.0, -1.0), (1.0, 1.0, 1.0))
+    X = I.reference_grid(g)
+    B0 = I.abc_field(X)
+    sim = make_sim(mr, g, X, B0)
+    sim.step(20, I.stable_dt(B0, g))
+    x = sim.get_fields(x=True)["x"].cpu().numpy()
+    assert np.abs(x - X).max() < 1e-13
+    assert sim.diagnostics()["max_jxb"] < 1e-11
+
+
+@pytest.mark.parametrize("variant", ["auto", "generic"])
+def test_fp32_variant_within_1e5_of_fp64(mr, variant):
+    """fp32 storage+arithmetic (displacement storage, Q15) against the fp64 GPU run and the fp64 oracle."""
+    cfg = I.scaled(I.CONFIGS["C5"], (64, 64, 64))
+    g = cfg.grid
+    x0, B0, dt = I.make(cfg)
+    s64 = make_sim(mr, g, x0, B0, "f64", variant)
+    s32 = make_sim(mr, g, x0, B0, "f32", variant)
+    s64.step(100, dt)
+    s32.step(100, dt)
+    x64 = s64.get_fields(x=True)["x"].cpu().numpy()
+    x32 = s32.get_fields(x=True)["x"].double().cpu().numpy()
+    assert nrel(x32, x64) < TOL_F32
+    assert nrel(x32 - x0, x64 - x0) < 1e-3      # even on the displacement itself
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 100)
+    assert nrel(x64, ref) < TOL_100
+    f32, f64 = fields_np(s32, "mimetic"), fields_np(s64, "mimetic")
+    assert nrel(f32["B"], f64["B"]) < TOL_F32
+    assert nrel(f32["J"], f64["J"]) < 1e-3      # J is a difference quotient: eps/h amplification
+    d32, d64 = s32.diagnostics(), s64.diagnostics()
+    assert d32["energy"] == pytest.approx(d64["energy"], rel=TOL_F32)
+
+
+def test_host_buffer_entry_points_round_trip(mr):
+    g, x0, B0, dt = case("ragged")
+    sim = mr.Relaxation(g.n, g.lo, g.hi)
+    sim.set_B0(torch.from_numpy(B0).pin_memory())
+    sim.set_x(torch.from_numpy(np.ascontiguousarray(x0)))          # pageable host memory also works
+    sim.step(3, dt)
+    out = sim.get_fields(x=True, B=True, J=True, host=True)
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 3)
+    B, J, _, _ = mro.fields(g.n, g.lo, g.hi, ref, B0)
+    assert nrel(out["x"].numpy(), ref) < TOL_STEP
+    assert nrel(out["B"].numpy(), B) < 1e-11
+    assert nrel(out["J"].numpy(), J) < 1e-10
+
+
+def test_error_paths_on_device(mr):
+    g, x0, B0, dt = case("C1")
+    sim = mr.Relaxation(g.n, g.lo, g.hi)
+    with pytest.raises(mr.MrError) as e:
+        sim.step(1, dt)
+    assert e.value.status == mr.MR_ERR_STATE
+    sim.set_B0(dev(B0))
+    with pytest.raises(mr.MrError) as e:
+        sim.step(1, -1.0)
+    assert e.value.status == mr.MR_ERR_INVALID_ARG
+    bad = np.array(x0)
+    bad[0, 0, 3, 3] += 0.1                                         # a boundary node off the reference grid
+    with pytest.raises(mr.MrError) as e:
+        sim.set_x(dev(bad))
+    assert e.value.status == mr.MR_ERR_INVALID_ARG
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), x0) < 1e-15      # state unchanged
+    folded = np.array(x0)
+    folded[0, 10, 8, 8] += 5.0                                     # folds the grid: det <= 0
+    sim.set_x(dev(folded))
+    with pytest.raises(mr.NumericError):
+        sim.step(1, dt)
+    with pytest.raises(mr.NumericError):                           # sticky until mr_set_x
+        sim.step(1, dt)
+    with pytest.raises(mr.NumericError):
+        mro.step(g.n, g.lo, g.hi, folded, B0, dt, 1)               # the oracle agrees that this is a failure
+    sim.set_x(dev(x0))
+    sim.step(1, dt)
+    wrong = torch.zeros((3, 4, 4, 4), device="cuda", dtype=torch.float64)
+    with pytest.raises(mr.MrError):
+        sim.set_B0(wrong)
+
+
+def test_zero_steps_is_a_no_op(mr):
+    g, x0, B0, dt = case("C1")
+    sim = make_sim(mr, g, x0, B0)
+    sim.step(0, dt)
+    assert np.array_equal(sim.get_fields(x=True)["x"].cpu().numpy(), x0)
+
+
+def test_full_size_config4_one_step_matches_oracle(mr):
+    """BASELINE configs[3] at full size (256x256x512, the bench workload and launch configuration), initial grid
+    smoothly displaced so that every term is exercised: x after one step and the diagnostics against the oracle
+    on the WHOLE grid (the oracle needs a few seconds per step with all host threads)."""
+    cfg = I.CONFIGS["C4"]
+    g = cfg.grid
+    _, B0, dt = I.make(cfg)
+    x0 = I.displaced_grid(g, 0.3, seed=11)
+    sim = make_sim(mr, g, x0, B0)
+    d = sim.diagnostics()
+    sim.step(1, dt)
+    x1 = sim.get_fields(x=True, host=True)["x"].numpy()
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 1)
+    assert nrel(x1, ref) < TOL_STEP
+    moved = np.abs(ref - x0).max()
+    assert np.abs(x1 - ref).max() < 1e-10 * moved + 1e-15 * np.abs(ref).max()
+    o = mro.diagnostics(g.n, g.lo, g.hi, x0, B0)
+    for k in ("energy", "max_jxb", "xi", "min_det"):
+        assert d[k] == pytest.approx(o[k], rel=TOL_STEP), k
