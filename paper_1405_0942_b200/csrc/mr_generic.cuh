@@ -12,6 +12,10 @@ struct DomainP {
     double h[3];
 };
 
+// X_a = lo_a + idx*h_a evaluated as a separately rounded product and sum (no FMA contraction), so that the
+// reference grid is bit-identical to the host-side definition lo + idx*h.
+__device__ __forceinline__ double ref_coord(double lo, double h, int idx) { return __dadd_rn(lo, __dmul_rn((double)idx, h)); }
+
 __device__ __forceinline__ bool node_of_thread(int nx, int ny, int nz, int& i, int& j, int& k)
 {
     i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -35,7 +39,7 @@ __global__ void k_import_x(const T* __restrict__ x, T* __restrict__ xi, GridP<T>
     bool off = false;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double X = d.lo[c] + (double)idx[c] * d.h[c];
+        const double X = ref_coord(d.lo[c], d.h[c], idx[c]);
         double v = (double)x[c * N + q] - X;
         if (bnd) {
             if (!(fabs(v) <= 1e-6 * d.h[c])) off = true;
@@ -73,7 +77,7 @@ __global__ void k_fields(const T* __restrict__ xi, const T* __restrict__ b, Grid
     if (x_out) {
         const int idx[3] = { i, j, k };
 #pragma unroll
-        for (int c = 0; c < 3; ++c) x_out[c * N + q] = (T)(d.lo[c] + (double)idx[c] * d.h[c] + (double)xi[c * g.comp + p]);
+        for (int c = 0; c < 3; ++c) x_out[c * N + q] = (T)__dadd_rn(ref_coord(d.lo[c], d.h[c], idx[c]), (double)xi[c * g.comp + p]);
     }
     if (!B_out && !J_out) return;
     const bool bnd = i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1;

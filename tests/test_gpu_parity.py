@@ -266,7 +266,7 @@ def test_error_paths_on_device(mr):
         sim.step(1, dt)
     with pytest.raises(mr.NumericError):                           # sticky until mr_set_x
         sim.step(1, dt)
-    with pytest.raises(mr.NumericError):
+    with pytest.raises(mro.NumericError):
         mro.step(g.n, g.lo, g.hi, folded, B0, dt, 1)               # the oracle agrees that this is a failure
     sim.set_x(dev(x0))
     sim.step(1, dt)
