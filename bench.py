@@ -45,13 +45,18 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def recorded_traffic(workload):
-    """dram bytes per launch from the committed ncu --set full capture (profiles/traffic.json), or None."""
+def recorded_traffic(workload, kernel):
+    """dram bytes per launch of this step kernel from the committed ncu --set full capture (profiles/traffic.csv,
+    written by hand from the summary it names), or None if this variant has not been captured."""
+    import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload, {}).get("dram_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["kernel"] == kernel:
+                    return float(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -251,7 +256,7 @@ def run_ours(args):
     launch_ms = ms / max(launches, 1)
     achieved = BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": recorded_traffic(cfg.name), "peak_source": peak_src, "kernel": variant,
+                "traffic": recorded_traffic(cfg.name, variant), "peak_source": peak_src, "kernel": variant,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE[dtype] * nodes, "launch_ms": launch_ms}
 
     # ---- end to end through the host-buffer entry points: H2D of x, one step, D2H of x, every step ----
