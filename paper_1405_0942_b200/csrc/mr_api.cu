@@ -10,6 +10,7 @@
 #include "mr_common.cuh"
 #include "mr_generic.cuh"
 #include "mr_stream.cuh"
+#include "mr_pair.cuh"
 
 using namespace mr;
 
@@ -71,9 +72,10 @@ struct mr_ctx {
     int64_t steps;
     int64_t launches;
     int sm_count;
-    int force_variant;  // 0 auto, 1 generic, 2 stream
+    int force_variant;  // 0 auto, 1 generic, 2 stream, 3 pair
     const char* variant;
-    StreamPlan plan;    // TMA descriptors etc. for the streaming kernel (mr_stream.cuh)
+    StreamPlan plan;    // TMA descriptors etc. for the first streaming kernel (mr_stream.cuh)
+    StreamPlan plan2;   // ... and for the register-paired streaming kernel (mr_pair.cuh), the default
     std::string err;
 
     void* xi(int w) const { return ws + L.off_xi[w]; }
@@ -210,14 +212,17 @@ mr_status launch_generic_step(mr_ctx* c, double dt, mr_operator op)
 template <typename T>
 mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
 {
-    const bool use_stream = op == MR_OP_MIMETIC && c->force_variant != 1 && c->plan.usable;
-    if (c->force_variant == 2 && !use_stream)
-        return fail(c, MR_ERR_INVALID_ARG, "mr_step: the streaming kernel was forced but does not take this grid/operator");
-    c->variant = use_stream ? c->plan.name : (op == MR_OP_MIMETIC ? "generic_mimetic" : "generic_direct");
+    const bool mim = op == MR_OP_MIMETIC;
+    const bool use_pair = mim && (c->force_variant == 0 || c->force_variant == 3) && c->plan2.usable;
+    const bool use_stream = mim && !use_pair && (c->force_variant == 0 || c->force_variant == 2) && c->plan.usable;
+    if ((c->force_variant == 2 && !use_stream) || (c->force_variant == 3 && !use_pair))
+        return fail(c, MR_ERR_INVALID_ARG, "mr_step: a streaming kernel was forced but does not take this grid/operator");
+    c->variant = use_pair ? c->plan2.name : use_stream ? c->plan.name : (mim ? "generic_mimetic" : "generic_direct");
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     for (int64_t s = 0; s < n; ++s) {
-        if (use_stream) {
-            cudaError_t e = launch_stream_step<T>(c->plan, c->cur, (T)(dt * c->gamma), c->flag(), c->stream);
+        if (use_pair || use_stream) {
+            cudaError_t e = use_pair ? launch_pair_step<T>(c->plan2, c->cur, (T)(dt * c->gamma), c->flag(), c->stream)
+                                     : launch_stream_step<T>(c->plan, c->cur, (T)(dt * c->gamma), c->flag(), c->stream);
             if (e != cudaSuccess) return cuda_fail(c, "streaming step launch", e);
             c->launches++;
         } else {
@@ -344,6 +349,10 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
         c->plan.usable = false;
         c->plan.why = why;
     }
+    if (!build_pair_plan(&c->plan2, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+        c->plan2.usable = false;
+        c->plan2.why = why;
+    }
     *out = c;
     return MR_OK;
 }
@@ -445,6 +454,7 @@ extern "C" mr_status mr_set_variant(mr_ctx* ctx, const char* name)
     if (!std::strcmp(name, "auto")) ctx->force_variant = 0;
     else if (!std::strcmp(name, "generic")) ctx->force_variant = 1;
     else if (!std::strcmp(name, "stream")) ctx->force_variant = 2;
-    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto, generic or stream");
+    else if (!std::strcmp(name, "pair")) ctx->force_variant = 3;
+    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto, generic, stream or pair");
     return MR_OK;
 }
