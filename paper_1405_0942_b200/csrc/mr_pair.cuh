@@ -18,6 +18,8 @@
 // innermost start coordinate 16-byte aligned, the right one is padded so that the row stride is 2 (mod 4)
 // doubles -- conflict-free column access.
 #pragma once
+#include <type_traits>
+
 #include "mr_stream.cuh"
 
 namespace mr {
@@ -59,14 +61,25 @@ __device__ __forceinline__ void face_fix(const T* __restrict__ f, unsigned edge,
     }
 }
 
-// D = det dF, 1/D, B = dF b / D (Eq. 2.1) from a finished dF (diagonal 2h not yet added)
+// Area vectors of the three index surfaces through a node, n_q = dF_{q+1} x dF_{q+2} (columns of dF; un-normalised
+// Eq. 2.5/2.6 -- the vector sum of the four triangles), D = det dF = dF_0 . n_0, 1/D and B = dF b / D (Eq. 2.1).
+// dF comes in without the 2h diagonal.
 template <typename T, int CSB>
-__device__ __forceinline__ void push_forward(T (&dF)[3][3], const T* __restrict__ bs, const T (&twoh)[3], T (&B)[3], T& inv,
-                                             bool& ok, bool in_dom)
+__device__ __forceinline__ void push_forward_n(T (&dF)[3][3], const T* __restrict__ bs, const T (&twoh)[3], T (&n)[3][3], T (&B)[3],
+                                               T& inv, bool& ok, bool in_dom)
 {
 #pragma unroll
     for (int c = 0; c < 3; ++c) dF[c][c] += twoh[c];
-    const T D = det3(dF);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const int q1 = (q + 1) % 3, q2 = (q + 2) % 3;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+            n[q][c] = dF[c1][q1] * dF[c2][q2] - dF[c2][q1] * dF[c1][q2];
+        }
+    }
+    const T D = dF[0][0] * n[0][0] + dF[1][0] * n[0][1] + dF[2][0] * n[0][2];
     ok = ok && (positive_finite(D) || !in_dom);
     inv = fast_rcp(D);
     const T b0 = bs[0] * inv, b1 = bs[CSB] * inv, b2 = bs[2 * CSB] * inv;
@@ -74,27 +87,24 @@ __device__ __forceinline__ void push_forward(T (&dF)[3][3], const T* __restrict_
     for (int c = 0; c < 3; ++c) B[c] = dF[c][0] * b0 + dF[c][1] * b1 + dF[c][2] * b2;
 }
 
-// xi += s (dF chat) x B, chat_p = eps_pqr dB_q . dF_r (closed form of Eqs. 2.3-2.7, Eq. 1.5); dB[a][c] = delta_a B_c
+// acc = n x v  /  acc += n x v, as chains of fused multiply-adds
 template <typename T>
-__device__ __forceinline__ void relax_node(const T (&dB)[3][3], const T (&dF)[3][3], const T (&Bc)[3], T s, bool doit, T (&x)[3],
-                                           bool& ok)
+__device__ __forceinline__ void cross_set(const T (&n)[3], const T (&v)[3], T (&acc)[3])
 {
-    T ch[3];
 #pragma unroll
-    for (int p = 0; p < 3; ++p) {
-        const int q = (p + 1) % 3, r = (p + 2) % 3;
-        ch[p] = dB[q][0] * dF[0][r] + dB[q][1] * dF[1][r] + dB[q][2] * dF[2][r]
-              - dB[r][0] * dF[0][q] - dB[r][1] * dF[1][q] - dB[r][2] * dF[2][q];
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        acc[c] = fma(n[c1], v[c2], -(n[c2] * v[c1]));
     }
-    T J[3], u[3];
+}
+template <typename T>
+__device__ __forceinline__ void cross_acc(const T (&n)[3], const T (&v)[3], T (&acc)[3])
+{
 #pragma unroll
-    for (int c = 0; c < 3; ++c) J[c] = dF[c][0] * ch[0] + dF[c][1] * ch[1] + dF[c][2] * ch[2];
-    cross3(J, Bc, u);
-    const T n0 = x[0] + s * u[0], n1 = x[1] + s * u[1], n2 = x[2] + s * u[2];
-    ok = ok && (is_finite(n0 + n1 + n2) || !doit);
-    x[0] = doit ? n0 : x[0];
-    x[1] = doit ? n1 : x[1];
-    x[2] = doit ? n2 : x[2];
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        acc[c] = fma(-n[c2], v[c1], fma(n[c1], v[c2], acc[c]));
+    }
 }
 
 template <typename T, int TY, int R, int RB>
@@ -123,25 +133,23 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
 
     // ---- TMA producer: lane 0 of the last warp (one without a ring node); a slot is refilled once its plane is dead ----
     const bool producer = tid == (NT - 1) * 32;
-    int next_x = pfirst, next_b = bfirst;
-    auto refill = [&](int dead_x, int dead_b) {
-        for (; next_x <= plast && next_x - R <= dead_x; ++next_x) {
-            const uint32_t s = (uint32_t)((next_x - pfirst) % R);
-            ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES);
-            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, next_x, 0, bar_x + 8u * s);
-        }
-        for (; next_b <= blast && next_b - RB <= dead_b; ++next_b) {
-            const uint32_t s = (uint32_t)((next_b - bfirst) % RB);
-            ptx::mbar_expect_tx(bar_b + 8u * s, L::BBOX_BYTES);
-            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, next_b, 0, bar_b + 8u * s);
-        }
+    auto load_x = [&](int p, uint32_t s) {
+        ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES);
+        ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, p, 0, bar_x + 8u * s);
+    };
+    auto load_b = [&](int p, uint32_t s) {
+        ptx::mbar_expect_tx(bar_b + 8u * s, L::BBOX_BYTES);
+        ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, p, 0, bar_b + 8u * s);
     };
     if (producer) {
         for (int s = 0; s < R + RB; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
         ptx::fence_mbar_init();
     }
     __syncthreads();
-    if (producer) refill(pfirst - 1, bfirst - 1);
+    if (producer) {   // the first R xi planes and RB b planes
+        for (int p = pfirst; p <= min(plast, pfirst + R - 1); ++p) load_x(p, (uint32_t)(p - pfirst));
+        for (int p = bfirst; p <= min(blast, bfirst + RB - 1); ++p) load_b(p, (uint32_t)(p - bfirst));
+    }
 
     auto wait_x = [&](int p) { const int q = p - pfirst; ptx::mbar_wait(bar_x + 8u * (uint32_t)(q % R), (uint32_t)((q / R) & 1)); };
     auto wait_b = [&](int p) { const int q = p - bfirst; ptx::mbar_wait(bar_b + 8u * (uint32_t)(q % RB), (uint32_t)((q / RB) & 1)); };
@@ -183,13 +191,14 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
     }
 
     // stage A of plane p at one node with every operand from shared memory (prologue only)
-    auto A_from_smem = [&](int p, int n, T(&dF)[3][3], T(&B)[3], T& inv, bool& ok) {
+    auto A_from_smem = [&](int p, int n, T(&nv)[3][3], T(&B)[3], T& inv, bool& ok) {
         const T* pc = xplane(p) + ox[n];
         const T *pa, *pb;
         T ca, cb, cc;     // on a k face: dk = ca * pa + cb * pb + cc * pc
         if (p == 0) { pa = xplane(1) + ox[n]; pb = xplane(2) + ox[n]; ca = T(4); cb = T(-1); cc = T(-3); }
         else if (p == nz - 1) { pa = xplane(p - 1) + ox[n]; pb = xplane(p - 2) + ox[n]; ca = T(-4); cb = T(1); cc = T(3); }
         else { pa = xplane(p + 1) + ox[n]; pb = xplane(p - 1) + ox[n]; ca = T(1); cb = T(-1); cc = T(0); }
+        T dF[3][3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             dF[c][0] = pc[c * CSX + 1] - pc[c * CSX - 1];
@@ -197,7 +206,7 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
             dF[c][2] = (p == 0 || p == nz - 1) ? ca * pa[c * CSX] + cc * pc[c * CSX] + cb * pb[c * CSX] : pa[c * CSX] - pb[c * CSX];
         }
         if (edge[n]) face_fix<T, BW, CSX>(pc, edge[n], dF);
-        push_forward<T, CSB>(dF, bplane(p) + ob[n], twoh, B, inv, ok, dom[n]);
+        push_forward_n<T, CSB>(dF, bplane(p) + ob[n], twoh, nv, B, inv, ok, dom[n]);
     };
     auto store_B = [&](int p, int n, const T(&B)[3]) {
         T* d = sB + (p & 1) * L::BSLOT + oB[n];
@@ -208,11 +217,12 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
 
     bool ok = true;
     // running ring positions of the xi planes k+1, k+2 and the b plane k+1 of the main loop
-    int sl1 = (k0 + 1 - pfirst) % R, sl2 = (k0 + 2 - pfirst) % R;
+    int sl0 = (k0 - pfirst) % R, sl1 = (k0 + 1 - pfirst) % R, sl2 = (k0 + 2 - pfirst) % R;
     uint32_t par2 = (uint32_t)(((k0 + 2 - pfirst) / R) & 1);
     int slb = (k0 + 1 - bfirst) % RB;
     uint32_t parb = (uint32_t)(((k0 + 1 - bfirst) / RB) & 1);
     auto advance = [&]() {
+        sl0 = sl1;
         sl1 = sl2;
         if (++sl2 == R) { sl2 = 0; par2 ^= 1u; }
         if (++slb == RB) { slb = 0; parb ^= 1u; }
@@ -240,140 +250,196 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
     const int gi = i0 + lane, gja = j0 + tj[0];
     const bool in_x = gi > 0 && gi < a.nx - 1;
     const bool in_xy0 = in_x && gja > 0 && gja < a.ny - 1, in_xy1 = in_x && gja + 1 < a.ny - 1;
-    const unsigned edges = edge[0] | edge[1];
-    T X[3][3][3];        // own xi at planes k, k+1, k+2 (rotating), per node (pair + ring node)
-    T Bq[3][2][3];       // own B at planes k-1, k, k+1 (rotating)
-    T dFq[2][2][3][3];   // dF at planes k, k+1 (rotating)
-    T invq[2][2];
-#pragma unroll
-    for (int n = 0; n < 3; ++n) {
-        const T* pa = xplane(k0) + ox[n];
-        const T* pb = xplane(min(k0 + 1, nz - 1)) + ox[n];
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            X[0][n][c] = pa[c * CSX];
-            X[1][n][c] = pb[c * CSX];
-            X[2][n][c] = T(0);
-        }
-    }
+    // Per-plane state of the pair, two sets used in turn (the loop is unrolled twice, so no register moves):
+    //   nq    area vectors n_0, n_1, n_2 of the plane      invq  1 / det dF
+    //   Bq    own B of the plane                            Wq    n_2(plane) x B(plane - 1), the lower half of the
+    //   Xq    own xi of the planes k+1, k+2                       k-loop term n_2 x (B(k+1) - B(k-1))
+    T nq[2][2][3][3], invq[2][2], Bq[2][2][3], Wq[2][2][3], Xq[2][2][3];
 #pragma unroll
     for (int n = 0; n < 2; ++n) {
+        const T* pb = xplane(min(k0 + 1, nz - 1)) + ox[n];
+        T Bl[3] = { T(0), T(0), T(0) };
+        if (k0 > 0) {
+            T nt[3][3], it;
+            A_from_smem(k0 - 1, n, nt, Bl, it, ok);
+        }
+        A_from_smem(k0, n, nq[0][n], Bq[0][n], invq[0][n], ok);
+        store_B(k0, n, Bq[0][n]);
+        cross_set(nq[0][n][2], Bl, Wq[0][n]);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            Bq[0][n][c] = T(0);
-            Bq[2][n][c] = T(0);
+            Xq[0][n][c] = pb[c * CSX];
+            Xq[1][n][c] = T(0);
         }
-        if (k0 > 0) {
-            T dFt[3][3], it;
-            A_from_smem(k0 - 1, n, dFt, Bq[0][n], it, ok);
-        }
-        A_from_smem(k0, n, dFq[0][n], Bq[1][n], invq[0][n], ok);
-        store_B(k0, n, Bq[1][n]);
-        invq[1][n] = T(0);
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int q = 0; q < 3; ++q) dFq[1][n][c][q] = T(0);
     }
     if (ring) {
-        T dF[3][3], B[3], inv;
-        A_from_smem(k0, 2, dF, B, inv, ok);
+        T nt[3][3], B[3], inv;
+        A_from_smem(k0, 2, nt, B, inv, ok);
         store_B(k0, 2, B);
     }
     ptx::cta_sync();
-    if (producer) refill(k0, k0);
+    if (producer) {   // planes < k0 of xi and <= k0 of b are dead: top the rings up to k0-1+R resp. k0+RB
+        for (int p = pfirst + R; p <= min(plast, k0 - 1 + R); ++p) load_x(p, (uint32_t)((p - pfirst) % R));
+        for (int p = bfirst + RB; p <= min(blast, k0 + RB); ++p) load_b(p, (uint32_t)((p - bfirst) % RB));
+    }
     T* po = out + (long long)k0 * a.plane + (long long)gja * a.pitch + gi;
     const bool st0 = gi < a.nx && gja < a.ny, st1 = gi < a.nx && gja + 1 < a.ny;
-
-    for (int kb = k0; kb < k1; kb += 6) {
+    // a tile is "plain" when neither it nor its halo-1 ring touches a face of the domain: no one-sided differences,
+    // no masks; the two instantiations of the main loop differ only in that
+    const bool plain = i0 > 0 && i0 + TX <= a.nx - 2 && j0 > 0 && j0 + TY <= a.ny - 2;
+    // the main loop takes the planes k0 .. kend-1, each with a stage A of plane k+1; the top plane nz-1 (line-tied,
+    // nothing above it) is copied through from its slot afterwards
+    const int kend = min(k1, nz - 1);
+    auto run = [&](auto plain_c) {
+        constexpr bool PLAIN = decltype(plain_c)::value;
+        for (int kb = k0; kb < kend; kb += 2) {
 #pragma unroll
-        for (int u = 0; u < 6; ++u) {
-            const int k = kb + u;
-            if (k >= k1) break;
-            T(&x0)[3][3] = X[u % 3];
-            T(&x1)[3][3] = X[(u + 1) % 3];
-            T(&x2)[3][3] = X[(u + 2) % 3];
-            T(&Bm)[2][3] = Bq[u % 3];
-            T(&Bc)[2][3] = Bq[(u + 1) % 3];
-            T(&Bp)[2][3] = Bq[(u + 2) % 3];
-            T(&dFc)[2][3][3] = dFq[u % 2];
-            T(&dFn)[2][3][3] = dFq[(u + 1) % 2];
-            if (k + 1 <= nz - 1) {
-                // ---- stage A of plane k+1 at the pair ----
-                T dk[2][3];
-                if (k + 2 <= nz - 1) ptx::mbar_wait(bar_x + 8u * (uint32_t)sl2, par2);
-                column_dk(k, 0, x0[0], x1[0], x2[0], dk[0]);
-                column_dk(k, 1, x0[1], x1[1], x2[1], dk[1]);
-                const T* f = sx + sl1 * L::SLOTX + ox[0];
+            for (int u = 0; u < 2; ++u) {
+                const int k = kb + u;
+                if (k >= kend) break;
+                T(&ncur)[2][3][3] = nq[u];
+                T(&nnew)[2][3][3] = nq[u ^ 1];
+                T(&Bc)[2][3] = Bq[u];
+                T(&Bn)[2][3] = Bq[u ^ 1];
+                T(&x1)[2][3] = Xq[u];
+                T(&x2)[2][3] = Xq[u ^ 1];
+                const bool inner_k = k > 0;          // (k <= nz-2 inside this loop)
+                const T* f0 = sx + sl0 * L::SLOTX + ox[0];
+                T x0[2][3];                           // own xi of plane k (re-read: plane k stays in its slot)
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    const T* fc = f + c * CSX;
-                    dFn[0][c][0] = fc[1] - fc[-1];
-                    dFn[1][c][0] = fc[BW + 1] - fc[BW - 1];
-                    dFn[0][c][1] = x1[1][c] - fc[-BW];
-                    dFn[1][c][1] = fc[2 * BW] - x1[0][c];
-                    dFn[0][c][2] = dk[0][c];
-                    dFn[1][c][2] = dk[1][c];
+                    x0[0][c] = f0[c * CSX];
+                    x0[1][c] = f0[c * CSX + BW];
                 }
-                if (edges) {
-                    if (edge[0]) face_fix<T, BW, CSX>(f, edge[0], dFn[0]);
-                    if (edge[1]) face_fix<T, BW, CSX>(f + BW, edge[1], dFn[1]);
-                }
-                ptx::mbar_wait(bar_b + 8u * (uint32_t)slb, parb);
-                const T* bs = sb + slb * L::SLOTB + ob[0];
-                push_forward<T, CSB>(dFn[0], bs, twoh, Bp[0], invq[(u + 1) % 2][0], ok, dom[0]);
-                push_forward<T, CSB>(dFn[1], bs + BW, twoh, Bp[1], invq[(u + 1) % 2][1], ok, dom[1]);
-                store_B(k + 1, 0, Bp[0]);
-                store_B(k + 1, 1, Bp[1]);
-                if (ring) {
-                    // ---- stage A of plane k+1 at the ring node ----
-                    T dkr[3], dF[3][3], B[3], inv;
-                    column_dk(k, 2, x0[2], x1[2], x2[2], dkr);
-                    const T* fr = sx + sl1 * L::SLOTX + ox[2];
+                T DJ[2][3];     // D J = sum_q n_q x delta_q B (closed form of Eqs. 2.3-2.7), built up in two parts
+                if (inner_k) {
+                    // ---- in-plane part of D J of plane k: n_0 x delta_i B + n_1 x delta_j B ----
+                    const T* g = sB + (k & 1) * L::BSLOT + oB[0];
+                    T dBi[2][3], dBj[2][3];
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
-                        dF[c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
-                        dF[c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
-                        dF[c][2] = dkr[c];
+                        const T* gc = g + c * BCS;
+                        dBi[0][c] = gc[1] - gc[-1];
+                        dBi[1][c] = gc[BBW + 1] - gc[BBW - 1];
+                        dBj[0][c] = Bc[1][c] - gc[-BBW];
+                        dBj[1][c] = gc[2 * BBW] - Bc[0][c];
                     }
-                    if (edge[2]) face_fix<T, BW, CSX>(fr, edge[2], dF);
-                    push_forward<T, CSB>(dF, sb + slb * L::SLOTB + ob[2], twoh, B, inv, ok, dom[2]);
-                    store_B(k + 1, 2, B);
-                }
-            }
-            if (k > 0 && k < nz - 1) {
-                // ---- stage B of plane k at the pair ----
-                const T* g = sB + (k & 1) * L::BSLOT + oB[0];
-                T dB[2][3][3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const T* gc = g + c * BCS;
-                    dB[0][0][c] = gc[1] - gc[-1];
-                    dB[1][0][c] = gc[BBW + 1] - gc[BBW - 1];
-                    dB[0][1][c] = Bc[1][c] - gc[-BBW];
-                    dB[1][1][c] = gc[2 * BBW] - Bc[0][c];
-                    dB[0][2][c] = Bp[0][c] - Bm[0][c];
-                    dB[1][2][c] = Bp[1][c] - Bm[1][c];
+                    for (int n = 0; n < 2; ++n) {
+                        cross_set(ncur[n][0], dBi[n], DJ[n]);
+                        cross_acc(ncur[n][1], dBj[n], DJ[n]);
+                    }
                 }
-                relax_node(dB[0], dFc[0], Bc[0], a.dtg * invq[u % 2][0], in_xy0, x0[0], ok);
-                relax_node(dB[1], dFc[1], Bc[1], a.dtg * invq[u % 2][1], in_xy1, x0[1], ok);
+                {
+                    // ---- stage A of plane k+1 at the pair ----
+                    T dF[2][3][3];
+                    const T* f = sx + sl1 * L::SLOTX + ox[0];
+                    if (k + 2 <= nz - 1) {
+                        ptx::mbar_wait(bar_x + 8u * (uint32_t)sl2, par2);
+                        const T* f2 = sx + sl2 * L::SLOTX + ox[0];
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            x2[0][c] = f2[c * CSX];
+                            x2[1][c] = f2[c * CSX + BW];
+                            dF[0][c][2] = x2[0][c] - x0[0][c];
+                            dF[1][c][2] = x2[1][c] - x0[1][c];
+                        }
+                    } else {   // top face: 3 x(nz-1) - 4 x(nz-2) + x(nz-3); plane nz-3 is still in its slot
+                        const T* fm = xplane(k - 1) + ox[0];
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            dF[0][c][2] = T(3) * x1[0][c] - T(4) * x0[0][c] + fm[c * CSX];
+                            dF[1][c][2] = T(3) * x1[1][c] - T(4) * x0[1][c] + fm[c * CSX + BW];
+                        }
+                    }
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        const T* fc = f + c * CSX;
+                        dF[0][c][0] = fc[1] - fc[-1];
+                        dF[1][c][0] = fc[BW + 1] - fc[BW - 1];
+                        dF[0][c][1] = x1[1][c] - fc[-BW];
+                        dF[1][c][1] = fc[2 * BW] - x1[0][c];
+                    }
+                    if (!PLAIN) {
+                        if (edge[0]) face_fix<T, BW, CSX>(f, edge[0], dF[0]);
+                        if (edge[1]) face_fix<T, BW, CSX>(f + BW, edge[1], dF[1]);
+                    }
+                    ptx::mbar_wait(bar_b + 8u * (uint32_t)slb, parb);
+                    const T* bs = sb + slb * L::SLOTB + ob[0];
+                    push_forward_n<T, CSB>(dF[0], bs, twoh, nnew[0], Bn[0], invq[u ^ 1][0], ok, PLAIN || dom[0]);
+                    push_forward_n<T, CSB>(dF[1], bs + BW, twoh, nnew[1], Bn[1], invq[u ^ 1][1], ok, PLAIN || dom[1]);
+                    store_B(k + 1, 0, Bn[0]);
+                    store_B(k + 1, 1, Bn[1]);
+                    cross_set(nnew[0][2], Bc[0], Wq[u ^ 1][0]);
+                    cross_set(nnew[1][2], Bc[1], Wq[u ^ 1][1]);
+                    if (ring) {
+                        // ---- stage A of plane k+1 at the ring node (every operand from shared memory) ----
+                        T dFr[3][3], nr[3][3], B[3], inv;
+                        const T* fr = sx + sl1 * L::SLOTX + ox[2];
+                        const T* fr0 = sx + sl0 * L::SLOTX + ox[2];
+                        if (k + 2 <= nz - 1) {
+                            const T* fr2 = sx + sl2 * L::SLOTX + ox[2];
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) dFr[c][2] = fr2[c * CSX] - fr0[c * CSX];
+                        } else {
+                            const T* fm = xplane(k - 1) + ox[2];
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) dFr[c][2] = T(3) * fr[c * CSX] - T(4) * fr0[c * CSX] + fm[c * CSX];
+                        }
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            dFr[c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
+                            dFr[c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
+                        }
+                        if (!PLAIN && edge[2]) face_fix<T, BW, CSX>(fr, edge[2], dFr);
+                        push_forward_n<T, CSB>(dFr, sb + slb * L::SLOTB + ob[2], twoh, nr, B, inv, ok, PLAIN || dom[2]);
+                        store_B(k + 1, 2, B);
+                    }
+                }
+                if (inner_k) {
+                    // ---- k part of D J: n_2 x (B(k+1) - B(k-1)); u = gamma J x B (Eq. 1.5); xi += dt u inside ----
+#pragma unroll
+                    for (int n = 0; n < 2; ++n) {
+                        T uu[3];
+                        cross_acc(ncur[n][2], Bn[n], DJ[n]);
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) DJ[n][c] -= Wq[u][n][c];
+                        cross_set(DJ[n], Bc[n], uu);
+                        const bool doit = PLAIN || (n == 0 ? in_xy0 : in_xy1);
+                        const T sc = doit ? a.dtg * invq[u][n] : T(0);
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) x0[n][c] = fma(sc, uu[c], x0[n][c]);
+                        ok = ok && (is_finite(x0[n][0] + x0[n][1] + x0[n][2]) || !doit);
+                    }
+                }
+                if (PLAIN || st0) {
+                    po[0] = x0[0][0];
+                    po[a.comp] = x0[0][1];
+                    po[2 * a.comp] = x0[0][2];
+                }
+                if (PLAIN || st1) {
+                    po[a.pitch] = x0[1][0];
+                    po[a.comp + a.pitch] = x0[1][1];
+                    po[2 * a.comp + a.pitch] = x0[1][2];
+                }
+                po += a.plane;
+                ptx::cta_sync();
+                // the xi plane k and the b plane k+1 are dead now: their slots take the planes k+R and k+1+RB
+                if (producer) {
+                    if (k + R <= plast) load_x(k + R, (uint32_t)sl0);
+                    if (k + 1 + RB <= blast) load_b(k + 1 + RB, (uint32_t)slb);
+                }
+                advance();
             }
-            if (st0) {
-                po[0] = x0[0][0];
-                po[a.comp] = x0[0][1];
-                po[2 * a.comp] = x0[0][2];
-            }
-            if (st1) {
-                po[a.pitch] = x0[1][0];
-                po[a.comp + a.pitch] = x0[1][1];
-                po[2 * a.comp + a.pitch] = x0[1][2];
-            }
-            po += a.plane;
-            ptx::cta_sync();
-            // xi planes <= k+1 and b planes <= k+1 are dead now (own columns live in registers): refill their slots
-            if (producer) refill(k + 1, k + 1);
-            advance();
         }
+    };
+    if (plain) run(std::true_type{});
+    else run(std::false_type{});
+    if (k1 == nz) {
+        const T* pt = xplane(nz - 1) + ox[0];
+        T* pl = out + (long long)(nz - 1) * a.plane + (long long)gja * a.pitch + gi;
+        if (st0) { pl[0] = pt[0]; pl[a.comp] = pt[CSX]; pl[2 * a.comp] = pt[2 * CSX]; }
+        if (st1) { pl[a.pitch] = pt[BW]; pl[a.comp + a.pitch] = pt[CSX + BW]; pl[2 * a.comp + a.pitch] = pt[2 * CSX + BW]; }
     }
     if (!ok) atomicOr(a.flag, FLAG_NUMERIC);
 }
