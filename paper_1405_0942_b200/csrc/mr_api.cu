@@ -11,6 +11,8 @@
 #include "mr_generic.cuh"
 #include "mr_stream.cuh"
 #include "mr_pair.cuh"
+#include "mr_lean.cuh"
+#include "mr_park.cuh"
 
 using namespace mr;
 
@@ -72,10 +74,12 @@ struct mr_ctx {
     int64_t steps;
     int64_t launches;
     int sm_count;
-    int force_variant;  // 0 auto, 1 generic, 2 stream, 3 pair
+    int force_variant;  // 0 auto, 1 generic, 2 stream, 3 pair, 4 lean, 5 park
     const char* variant;
     StreamPlan plan;    // TMA descriptors etc. for the first streaming kernel (mr_stream.cuh)
-    StreamPlan plan2;   // ... and for the register-paired streaming kernel (mr_pair.cuh), the default
+    StreamPlan plan2;   // ... for the register-paired streaming kernel (mr_pair.cuh)
+    StreamPlan plan3;   // ... for the lean-state streaming kernel (mr_lean.cuh)
+    StreamPlan plan4;   // ... and for the TMEM-parked streaming kernel (mr_park.cuh), the default
     std::string err;
 
     void* xi(int w) const { return ws + L.off_xi[w]; }
@@ -213,16 +217,23 @@ template <typename T>
 mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
 {
     const bool mim = op == MR_OP_MIMETIC;
-    const bool use_pair = mim && (c->force_variant == 0 || c->force_variant == 3) && c->plan2.usable;
-    const bool use_stream = mim && !use_pair && (c->force_variant == 0 || c->force_variant == 2) && c->plan.usable;
-    if ((c->force_variant == 2 && !use_stream) || (c->force_variant == 3 && !use_pair))
+    const int fv = c->force_variant;
+    const bool use_park = mim && (fv == 0 || fv == 5) && c->plan4.usable;
+    const bool use_lean = mim && !use_park && (fv == 0 || fv == 4) && c->plan3.usable;
+    const bool use_pair = mim && !use_park && !use_lean && (fv == 0 || fv == 3) && c->plan2.usable;
+    const bool use_stream = mim && !use_park && !use_lean && !use_pair && (fv == 0 || fv == 2) && c->plan.usable;
+    if ((fv == 2 && !use_stream) || (fv == 3 && !use_pair) || (fv == 4 && !use_lean) || (fv == 5 && !use_park))
         return fail(c, MR_ERR_INVALID_ARG, "mr_step: a streaming kernel was forced but does not take this grid/operator");
-    c->variant = use_pair ? c->plan2.name : use_stream ? c->plan.name : (mim ? "generic_mimetic" : "generic_direct");
+    c->variant = use_park ? c->plan4.name : use_lean ? c->plan3.name : use_pair ? c->plan2.name : use_stream ? c->plan.name
+                 : (mim ? "generic_mimetic" : "generic_direct");
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     for (int64_t s = 0; s < n; ++s) {
-        if (use_pair || use_stream) {
-            cudaError_t e = use_pair ? launch_pair_step<T>(c->plan2, c->cur, (T)(dt * c->gamma), c->flag(), c->stream)
-                                     : launch_stream_step<T>(c->plan, c->cur, (T)(dt * c->gamma), c->flag(), c->stream);
+        if (use_park || use_lean || use_pair || use_stream) {
+            const T dtg = (T)(dt * c->gamma);
+            cudaError_t e = use_park ? launch_park_step<T>(c->plan4, c->cur, dtg, c->flag(), c->stream)
+                            : use_lean ? launch_lean_step<T>(c->plan3, c->cur, dtg, c->flag(), c->stream)
+                            : use_pair ? launch_pair_step<T>(c->plan2, c->cur, dtg, c->flag(), c->stream)
+                                       : launch_stream_step<T>(c->plan, c->cur, dtg, c->flag(), c->stream);
             if (e != cudaSuccess) return cuda_fail(c, "streaming step launch", e);
             c->launches++;
         } else {
@@ -353,6 +364,14 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
         c->plan2.usable = false;
         c->plan2.why = why;
     }
+    if (!build_lean_plan(&c->plan3, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+        c->plan3.usable = false;
+        c->plan3.why = why;
+    }
+    if (!build_park_plan(&c->plan4, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+        c->plan4.usable = false;
+        c->plan4.why = why;
+    }
     *out = c;
     return MR_OK;
 }
@@ -455,6 +474,8 @@ extern "C" mr_status mr_set_variant(mr_ctx* ctx, const char* name)
     else if (!std::strcmp(name, "generic")) ctx->force_variant = 1;
     else if (!std::strcmp(name, "stream")) ctx->force_variant = 2;
     else if (!std::strcmp(name, "pair")) ctx->force_variant = 3;
-    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto, generic, stream or pair");
+    else if (!std::strcmp(name, "lean")) ctx->force_variant = 4;
+    else if (!std::strcmp(name, "park")) ctx->force_variant = 5;
+    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto, generic, stream, pair, lean or park");
     return MR_OK;
 }

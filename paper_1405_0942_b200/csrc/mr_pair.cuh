@@ -446,7 +446,12 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
 
 // ----------------------------------------------------------------------------------------------- host side
 
-constexpr int kPTY = 16, kPR = 6, kPRB = 3;
+#ifndef MR_PTY
+#define MR_PTY 16
+#define MR_PR 6
+#define MR_PRB 3
+#endif
+constexpr int kPTY = MR_PTY, kPR = MR_PR, kPRB = MR_PRB;
 
 template <typename T>
 inline cudaError_t pair_set_smem(size_t bytes)

@@ -57,6 +57,7 @@ struct StreamPlan {
     CUtensorMap map_xi[2];
     CUtensorMap map_b;
     void* xi[2] = { nullptr, nullptr };
+    const void* b = nullptr;
     int tiles_x = 0, tiles_y = 0, nchunks = 0, chunk_len = 0;
     size_t smem_bytes = 0;
 };
