@@ -1,0 +1,517 @@
+// mr_duo.cuh -- the warp-specialised streaming step kernel for the mimetic operator (S1-S5 in one pass).
+//
+// ncu of the register-paired kernel (profiles/r1c): one CTA of 8 warps per SM, 255 registers, every pipe below 45 %
+// and the warps waiting on each other's latencies -- the kernel is bound by the number of nodes the register file
+// can keep in flight, not by HBM (the same TMA ring with the arithmetic stubbed out runs at 96 % of the measured
+// copy bandwidth).  This kernel splits the work of a node between two warps that hand the node's state over through
+// Tensor Memory (mr_tmem.cuh), so that 16 warps of 128 registers share the SM and the two roles run out of step:
+//
+//   A-warps (0..TY/2-1, lane = i, rows 2a and 2a+1; the first ones also carry a node of the halo-1 ring)
+//       plane p:  dF from the xi ring in shared memory (TMA), area vectors n_q (Eqs. 2.5/2.6), D = det dF,
+//                 B(p) = dF b / D (Eq. 2.1) -> shared B plane p % NB;   record(p) = n_0, n_1, n_2, s = dt gamma / D,
+//                 own xi(p) -> TMEM buffer p % NB;   bar.arrive FULL[p % NB]
+//   F-warps (TY/2..TY-1, same lanes and rows: the partner warp sits in the same TMEM lane quarter)
+//       plane t:  bar.sync FULL[(t+1) % NB];  D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x (B(t+1) - B(t-1))
+//                 (closed form of Eqs. 2.3-2.7) from record(t), the shared B plane t and the own B(t-1), B(t), B(t+1);
+//                 u = gamma J x B (Eq. 1.5);  xi+ = xi + dt u -> HBM;   bar.arrive FREE[t % NB]
+// The A-warps wait on FREE[p % NB] before they overwrite a buffer, so they run up to NB-1 planes ahead of the
+// F-warps; the xi / b rings are touched by the A-warps only and recycled behind a barrier of their own.
+// B, J, u never touch HBM: the algorithmic traffic is read xi + read b + write xi+ = 9 elements per node.
+#pragma once
+#include <type_traits>
+
+#include "mr_pair.cuh"
+#include "mr_tmem.cuh"
+
+namespace mr {
+
+template <typename T, int TY, int R, int RB, int NB>
+struct DuoLayout {
+    static_assert(TY % 2 == 0 && TY >= 8 && TY <= 16 && R >= 4 && RB >= 2 && NB >= 3, "tile / ring sizes");
+    static constexpr int TX = 32;
+    static constexpr int HXL = 16 / (int)sizeof(T), HXR = 2 * HXL;
+    static constexpr int BW = TX + HXL + HXR;
+    static constexpr int XH = TY + 4, BH = TY + 2;
+    static constexpr int CSX = BW * XH, CSB = BW * BH;
+    static constexpr int round128(int bytes) { return (bytes + 127) / 128 * 128; }
+    static constexpr int SLOTX = round128(3 * CSX * (int)sizeof(T)) / (int)sizeof(T);
+    static constexpr int SLOTB = round128(3 * CSB * (int)sizeof(T)) / (int)sizeof(T);
+    static constexpr uint32_t XBOX_BYTES = 3u * CSX * sizeof(T), BBOX_BYTES = 3u * CSB * sizeof(T);
+    static constexpr int BBW = TX + 2, BBH = TY + 2;
+    static constexpr int BCS = BBW * BBH;
+    static constexpr int BSLOT = round128(3 * BCS * (int)sizeof(T)) / (int)sizeof(T);
+    static constexpr int NAW = TY / 2, NWARPS = 2 * NAW, NTHREADS = NWARPS * 32;
+    static constexpr size_t OFF_X = 0;
+    static constexpr size_t OFF_B0 = OFF_X + (size_t)R * SLOTX * sizeof(T);
+    static constexpr size_t OFF_BB = OFF_B0 + (size_t)RB * SLOTB * sizeof(T);
+    static constexpr size_t OFF_BAR = OFF_BB + (size_t)NB * BSLOT * sizeof(T);
+    static constexpr size_t BYTES = OFF_BAR + (size_t)(R + RB) * 8 + 128;   // +128: base alignment slack
+};
+
+namespace ptx {
+__device__ __forceinline__ void named_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void named_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+}  // namespace ptx
+
+// The A-warp's share of stage A at one node: dF comes in without the 2h diagonal and leaves with it; n_0 = dF_1 x dF_2
+// (area vector of the jk index surface, Eqs. 2.5/2.6), D = det dF = dF_0 . n_0, inv = 1/D, B = dF b / D (Eq. 2.1).
+// n_1 and n_2 are formed by the F-warp from the columns of dF.
+template <typename T, int CSB>
+__device__ __forceinline__ void duo_push(T (&dF)[3][3], const T* __restrict__ bs, const T (&twoh)[3], T (&n0)[3], T (&B)[3], T& inv,
+                                         bool& ok, bool in_dom)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dF[c][c] += twoh[c];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        n0[c] = dF[c1][1] * dF[c2][2] - dF[c2][1] * dF[c1][2];
+    }
+    const T D = dF[0][0] * n0[0] + dF[1][0] * n0[1] + dF[2][0] * n0[2];
+    ok = ok && (positive_finite(D) || !in_dom);
+    inv = fast_rcp(D);
+    const T b0 = bs[0] * inv, b1 = bs[CSB] * inv, b2 = bs[2 * CSB] * inv;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) B[c] = dF[c][0] * b0 + dF[c][1] * b1 + dF[c][2] * b2;
+}
+
+template <typename T, int TY, int R, int RB, int NB>
+__global__ void __launch_bounds__(TY * 32, 1)
+k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, T* __restrict__ out,
+           const StreamArgs<T> a)
+{
+    using L = DuoLayout<T, TY, R, RB, NB>;
+    using W32 = tmem::Words<T>;
+    constexpr int TX = L::TX, NAW = L::NAW, BW = L::BW, CSX = L::CSX, CSB = L::CSB, BBW = L::BBW, BCS = L::BCS;
+    constexpr int NTH = L::NTHREADS;
+    constexpr int CW = 8 * W32::N;                  // words per TMEM chunk (8 values)
+    constexpr int REC = 2 * CW;                     // words per node record: {n0, n1, x0, x1 | n2, s, x2, -, -, -}
+    constexpr int PAIRCOLS = 2 * REC * NB;          // columns of one A/F warp pair
+    static_assert(((NAW + 3) / 4) * PAIRCOLS <= 512, "TMEM columns");
+    // named barriers, one of each kind per buffer: an A-warp may run NB-1 planes ahead of the slowest one
+    constexpr int BAR_FULL = 1, BAR_FREE = 1 + NB, BAR_A = 1 + 2 * NB;
+    static_assert(1 + 3 * NB <= 16, "named barriers");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t tm_base_s;
+    unsigned char* smem = smem_raw + ((128u - (ptx::smem_u32(smem_raw) & 127u)) & 127u);
+    const T* sx = reinterpret_cast<const T*>(smem + L::OFF_X);
+    const T* sb = reinterpret_cast<const T*>(smem + L::OFF_B0);
+    T* sB = reinterpret_cast<T*>(smem + L::OFF_BB);
+    const uint32_t sx_u32 = ptx::smem_u32(sx), sb_u32 = ptx::smem_u32(sb);
+    const uint32_t bar_x = ptx::smem_u32(smem + L::OFF_BAR), bar_b = bar_x + 8u * R;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool isA = warp < NAW;
+    const int widx = isA ? warp : warp - NAW;       // the A-warp and the F-warp of the same rows share widx
+    const int tile = blockIdx.x % a.ntiles, chunk = blockIdx.x / a.ntiles;
+    const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY;
+    const int nz = a.nz;
+    const int k0 = chunk * a.chunk_len, k1 = min(k0 + a.chunk_len, nz);
+    const int kend = min(k1, nz - 1);               // planes k0 .. kend-1 are finished here (and nz-1 carried through)
+    const int first_p = max(k0 - 1, 0);             // the A-warps form B of the planes first_p .. kend
+    const int pfirst = max(first_p - 1, 0), plast = min(kend + 1, nz - 1);   // xi planes this item touches
+    const int bfirst = first_p, blast = kend;                                // b planes
+
+    const bool producer = tid == (NAW - 1) * 32;
+    if (producer) {
+        for (int s = 0; s < R + RB; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
+        ptx::fence_mbar_init();
+    }
+    if (warp == 0) tmem::alloc<512>(&tm_base_s);
+    tmem::fence_before_sync();
+    __syncthreads();
+    tmem::fence_after_sync();
+    const uint32_t tm0 = tm_base_s + ((uint32_t)(32 * (widx & 3)) << 16) + (uint32_t)((widx >> 2) * PAIRCOLS);
+    auto rec_addr = [&](int buf, int n, int c) -> uint32_t { return tm0 + (uint32_t)((buf * 2 + n) * REC + c * CW); };
+
+    const int gi = i0 + lane, gja = j0 + 2 * widx;
+    const bool st[2] = { gi < a.nx && gja < a.ny, gi < a.nx && gja + 1 < a.ny };
+    const int oB0 = (2 * widx + 1) * BBW + (lane + 1);      // the pair's node 0 inside a shared B plane
+    bool ok = true;
+
+    if (isA) {
+        // =============================================== A-warps ===============================================
+        const T twoh[3] = { a.twoh[0], a.twoh[1], a.twoh[2] };
+        auto load_x = [&](int p) {
+            const uint32_t s = (uint32_t)((p - pfirst) % R);
+            ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES);
+            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, p, 0, bar_x + 8u * s);
+        };
+        auto load_b = [&](int p) {
+            const uint32_t s = (uint32_t)((p - bfirst) % RB);
+            ptx::mbar_expect_tx(bar_b + 8u * s, L::BBOX_BYTES);
+            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, p, 0, bar_b + 8u * s);
+        };
+        int next_x = pfirst, next_b = bfirst;                      // next planes to request (producer only)
+        auto refill = [&](int upto_x, int upto_b) {
+            for (const int last = min(upto_x, plast); next_x <= last; ++next_x) load_x(next_x);
+            for (const int last = min(upto_b, blast); next_b <= last; ++next_b) load_b(next_b);
+        };
+        if (producer) refill(pfirst + R - 1, bfirst + RB - 1);
+        auto wait_x = [&](int p) { const int q = p - pfirst; ptx::mbar_wait(bar_x + 8u * (uint32_t)(q % R), (uint32_t)((q / R) & 1)); };
+        auto wait_b = [&](int p) { const int q = p - bfirst; ptx::mbar_wait(bar_b + 8u * (uint32_t)(q % RB), (uint32_t)((q / RB) & 1)); };
+        auto xplane = [&](int p) -> const T* { return sx + ((p - pfirst) % R) * L::SLOTX; };
+        auto bplane = [&](int p) -> const T* { return sb + ((p - bfirst) % RB) * L::SLOTB; };
+
+        // nodes: 0, 1 = the pair (lane, 2 warp), (lane, 2 warp + 1); 2 = a node of the halo-1 ring (warps 0..2)
+        int ti2, tj2;
+        constexpr int NRINGW = 2 + (TY + 15) / 16;
+        static_assert(NRINGW < NAW, "the last A-warp (TMA producer) carries no ring node");
+        bool ring = warp < NRINGW;
+        if (warp == 0) { ti2 = lane; tj2 = -1; }
+        else if (warp == 1) { ti2 = lane; tj2 = TY; }
+        else {
+            ti2 = (lane >> 3) & 1 ? TX : -1;
+            tj2 = (lane & 7) + 8 * (lane >> 4) + 16 * (warp - 2);
+            if (tj2 >= TY) { ring = false; tj2 = 0; }
+        }
+        const int ox0 = (2 * warp + 2) * BW + (lane + L::HXL), ob0 = (2 * warp + 1) * BW + (lane + L::HXL);
+        const int ox2 = (tj2 + 2) * BW + (ti2 + L::HXL), ob2 = (tj2 + 1) * BW + (ti2 + L::HXL), oB2 = (tj2 + 1) * BBW + (ti2 + 1);
+        unsigned edge[3];
+        bool dom[3];
+        {
+            const int gis[3] = { gi, gi, i0 + ti2 }, gjs[3] = { gja, gja + 1, j0 + tj2 };
+#pragma unroll
+            for (int n = 0; n < 3; ++n) {
+                dom[n] = gis[n] >= 0 && gis[n] < a.nx && gjs[n] >= 0 && gjs[n] < a.ny && (n < 2 || ring);
+                edge[n] = !dom[n] ? 0u
+                    : (gis[n] == 0 ? 1u : 0u) | (gis[n] == a.nx - 1 ? 2u : 0u) | (gjs[n] == 0 ? 4u : 0u) | (gjs[n] == a.ny - 1 ? 8u : 0u);
+            }
+        }
+        const bool in_x = gi > 0 && gi < a.nx - 1;
+        const bool in_xy[2] = { in_x && gja > 0 && gja < a.ny - 1, in_x && gja + 1 < a.ny - 1 };
+        const bool plain = i0 > 0 && i0 + TX <= a.nx - 2 && j0 > 0 && j0 + TY <= a.ny - 2;
+
+        for (int p = pfirst; p <= min(first_p + 1, plast); ++p) wait_x(p);
+        if (first_p == 0 && plast >= 2) wait_x(2);          // the one-sided difference on the bottom face
+        T xc[2][3], xr[3];                                  // own xi(p-1) of the pair and of the ring node
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { xc[0][c] = T(0); xc[1][c] = T(0); xr[c] = T(0); }
+        if (first_p > 0) {
+            const T* f = xplane(first_p - 1);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                xc[0][c] = f[ox0 + c * CSX];
+                xc[1][c] = f[ox0 + c * CSX + BW];
+                xr[c] = f[ox2 + c * CSX];
+            }
+        }
+        auto runA = [&](auto plain_c) {
+            constexpr bool PLAIN = decltype(plain_c)::value;
+            int buf = first_p % NB;
+            // running ring positions: xi planes p-2 .. p+2 (slots sm2, sm1, s0, s1, s2), parity of the plane p+1, b plane p
+            int s0 = (first_p - pfirst) % R, s1 = (s0 + 1) % R, s2 = (s0 + 2) % R, sm1 = (s0 + R - 1) % R, sm2 = (s0 + R - 2) % R;
+            uint32_t par1 = (uint32_t)(((first_p + 1 - pfirst) / R) & 1);
+            int sb0 = 0;
+            uint32_t parb = 0u;
+#pragma unroll 1
+            for (int p = first_p; p <= kend; ++p) {
+                const T* f1 = sx + s0 * L::SLOTX;                     // xi plane p
+                const T* f2 = sx + s1 * L::SLOTX;                     // xi plane p+1
+                if (p + 1 <= plast) ptx::mbar_wait(bar_x + 8u * (uint32_t)s1, par1);
+                ptx::mbar_wait(bar_b + 8u * (uint32_t)sb0, parb);
+                const T* bs = sb + sb0 * L::SLOTB;
+                const bool inner_k = p > 0 && p < nz - 1;
+                T x1[2][3], dF[2][3][3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    x1[0][c] = f1[ox0 + c * CSX];
+                    x1[1][c] = f1[ox0 + c * CSX + BW];
+                }
+                if (p == 0) {                   // bottom face: -3 x(0) + 4 x(1) - x(2)
+                    const T* f3 = sx + s2 * L::SLOTX;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        dF[0][c][2] = T(4) * f2[ox0 + c * CSX] - T(3) * x1[0][c] - f3[ox0 + c * CSX];
+                        dF[1][c][2] = T(4) * f2[ox0 + c * CSX + BW] - T(3) * x1[1][c] - f3[ox0 + c * CSX + BW];
+                    }
+                } else if (p + 1 <= nz - 1) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        dF[0][c][2] = f2[ox0 + c * CSX] - xc[0][c];
+                        dF[1][c][2] = f2[ox0 + c * CSX + BW] - xc[1][c];
+                    }
+                } else {                        // top face: 3 x(nz-1) - 4 x(nz-2) + x(nz-3); plane nz-3 is still in its slot
+                    const T* fm = sx + sm2 * L::SLOTX;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        dF[0][c][2] = T(3) * x1[0][c] - T(4) * xc[0][c] + fm[ox0 + c * CSX];
+                        dF[1][c][2] = T(3) * x1[1][c] - T(4) * xc[1][c] + fm[ox0 + c * CSX + BW];
+                    }
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const T* fc = f1 + ox0 + c * CSX;
+                    dF[0][c][0] = fc[1] - fc[-1];
+                    dF[1][c][0] = fc[BW + 1] - fc[BW - 1];
+                    dF[0][c][1] = x1[1][c] - fc[-BW];
+                    dF[1][c][1] = fc[2 * BW] - x1[0][c];
+                }
+                if (!PLAIN) {
+                    if (edge[0]) face_fix<T, BW, CSX>(f1 + ox0, edge[0], dF[0]);
+                    if (edge[1]) face_fix<T, BW, CSX>(f1 + ox0 + BW, edge[1], dF[1]);
+                }
+                // the buffer p % NB (shared B plane and TMEM records) must have been read by the F-warps
+                if (p >= first_p + NB) {
+                    ptx::named_sync(BAR_FREE + buf, NTH);
+                    tmem::fence_after_sync();
+                }
+                T* Bd = sB + buf * L::BSLOT;
+#pragma unroll
+                for (int n = 0; n < 2; ++n) {
+                    T n0[3], Bn[3], inv;
+                    duo_push<T, CSB>(dF[n], bs + ob0 + n * BW, twoh, n0, Bn, inv, ok, PLAIN || dom[n]);
+                    T* d = Bd + oB0 + n * BBW;
+                    d[0] = Bn[0];
+                    d[BCS] = Bn[1];
+                    d[2 * BCS] = Bn[2];
+                    const T sn = (inner_k && (PLAIN || in_xy[n])) ? a.dtg * inv : T(0);
+                    // record(p) = columns 0, 1 of dF, xi_0, xi_1 | column 2 of dF, n_0, s, xi_2
+                    uint32_t w0[CW], w1[CW];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        W32::put(w0 + c * W32::N, dF[n][c][0]);
+                        W32::put(w0 + (3 + c) * W32::N, dF[n][c][1]);
+                        W32::put(w1 + c * W32::N, dF[n][c][2]);
+                        W32::put(w1 + (3 + c) * W32::N, n0[c]);
+                    }
+                    W32::put(w0 + 6 * W32::N, x1[n][0]);
+                    W32::put(w0 + 7 * W32::N, x1[n][1]);
+                    W32::put(w1 + 6 * W32::N, sn);
+                    W32::put(w1 + 7 * W32::N, x1[n][2]);
+                    if constexpr (CW == 16) { tmem::st16(rec_addr(buf, n, 0), w0); tmem::st16(rec_addr(buf, n, 1), w1); }
+                    else { tmem::st8(rec_addr(buf, n, 0), w0); tmem::st8(rec_addr(buf, n, 1), w1); }
+                }
+                if (ring && p >= k0 && p < kend) {
+                    // stage A at the ring node (planes k0 .. kend-1: the planes whose in-plane differences are taken)
+                    T dFr[3][3], nr[3], B[3], inv, xr1[3];
+                    const T* fr = f1 + ox2;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        xr1[c] = fr[c * CSX];
+                        dFr[c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
+                        dFr[c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
+                    }
+                    if (p == 0) {
+                        const T* f3 = sx + s2 * L::SLOTX;
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) dFr[c][2] = T(4) * f2[ox2 + c * CSX] - T(3) * xr1[c] - f3[ox2 + c * CSX];
+                    } else if (p + 1 <= nz - 1) {
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) dFr[c][2] = f2[ox2 + c * CSX] - xr[c];
+                    } else {
+                        const T* fm = sx + sm2 * L::SLOTX;
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) dFr[c][2] = T(3) * xr1[c] - T(4) * xr[c] + fm[ox2 + c * CSX];
+                    }
+                    if (!PLAIN && edge[2]) face_fix<T, BW, CSX>(fr, edge[2], dFr);
+                    duo_push<T, CSB>(dFr, bs + ob2, twoh, nr, B, inv, ok, PLAIN || dom[2]);
+                    T* d = Bd + oB2;
+                    d[0] = B[0];
+                    d[BCS] = B[1];
+                    d[2 * BCS] = B[2];
+                }
+                if (ring) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) xr[c] = f1[ox2 + c * CSX];
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { xc[0][c] = x1[0][c]; xc[1][c] = x1[1][c]; }
+                tmem::wait_st();
+                tmem::fence_before_sync();
+                ptx::named_arrive(BAR_FULL + buf, NTH);           // B(p) and record(p) are published
+                // every A-warp is done with the xi / b planes p: only the producer's warp waits for the others
+                if (warp == NAW - 1) {
+                    ptx::named_sync(BAR_A + buf, NAW * 32);
+                    if (producer) refill(p + R, p + RB);   // the slots of the planes <= p take the planes up to p + R / p + RB
+                } else {
+                    ptx::named_arrive(BAR_A + buf, NAW * 32);
+                }
+                if (++buf == NB) buf = 0;
+                sm2 = sm1; sm1 = s0; s0 = s1; s1 = s2;
+                if (s1 == 0) par1 ^= 1u;                          // the slot of the plane p+1 wrapped around
+                if (++s2 == R) s2 = 0;
+                if (++sb0 == RB) { sb0 = 0; parb ^= 1u; }
+            }
+        };
+        if (plain) runA(std::true_type{});
+        else runA(std::false_type{});
+    } else {
+        // =============================================== F-warps ===============================================
+        auto ownB = [&](int buf, T(&B)[2][3]) {
+            const T* g = sB + buf * L::BSLOT + oB0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                B[0][c] = g[c * BCS];
+                B[1][c] = g[c * BCS + BBW];
+            }
+        };
+        auto fetch = [&](int buf, int n, uint32_t(&w0)[CW], uint32_t(&w1)[CW]) {
+            if constexpr (CW == 16) { tmem::ld16(rec_addr(buf, n, 0), w0); tmem::ld16(rec_addr(buf, n, 1), w1); }
+            else { tmem::ld8(rec_addr(buf, n, 0), w0); tmem::ld8(rec_addr(buf, n, 1), w1); }
+        };
+        T Bm[2][3], Bc[2][3];                           // own B(t-1), B(t) of the pair
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { Bm[0][c] = T(0); Bm[1][c] = T(0); }
+        int buf = first_p % NB;                         // buffer of the plane t
+        if (k0 > 0) {
+            ptx::named_sync(BAR_FULL + buf, NTH);       // plane k0-1: only the own B is needed
+            ownB(buf, Bm);
+            ptx::named_arrive(BAR_FREE + buf, NTH);
+            if (++buf == NB) buf = 0;
+        }
+        ptx::named_sync(BAR_FULL + buf, NTH);           // plane k0
+        tmem::fence_after_sync();
+        ownB(buf, Bc);
+        T* po = out + (long long)k0 * a.plane + (long long)gja * a.pitch + gi;
+#pragma unroll 1
+        for (int t = k0; t < kend; ++t) {
+            const int bufn = buf + 1 == NB ? 0 : buf + 1;
+            uint32_t w0[CW], w1[CW];
+            fetch(buf, 0, w0, w1);                      // record(t) of node 0 (published with plane t)
+            ptx::named_sync(BAR_FULL + bufn, NTH);      // plane t+1
+            tmem::fence_after_sync();
+            T Bp[2][3];
+            ownB(bufn, Bp);
+            const T* g = sB + buf * L::BSLOT + oB0;
+#pragma unroll
+            for (int n = 0; n < 2; ++n) {
+                T dBi[3], dBj[3], dBk[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const T* gc = g + c * BCS + n * BBW;
+                    dBi[c] = gc[1] - gc[-1];
+                    dBj[c] = n == 0 ? Bc[1][c] - gc[-BBW] : gc[BBW] - Bc[0][c];
+                    dBk[c] = Bp[n][c] - Bm[n][c];
+                }
+                tmem::wait_ld(w0);
+                tmem::wait_ld(w1);
+                T c0[3], c1[3], c2[3], n0[3], n1[3], n2[3], x[3], DJ[3], uu[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    c0[c] = W32::get(w0 + c * W32::N);
+                    c1[c] = W32::get(w0 + (3 + c) * W32::N);
+                    c2[c] = W32::get(w1 + c * W32::N);
+                    n0[c] = W32::get(w1 + (3 + c) * W32::N);
+                }
+                x[0] = W32::get(w0 + 6 * W32::N);
+                x[1] = W32::get(w0 + 7 * W32::N);
+                x[2] = W32::get(w1 + 7 * W32::N);
+                const T s = W32::get(w1 + 6 * W32::N);
+                cross_set(c2, c0, n1);                  // n_1 = dF_2 x dF_0,  n_2 = dF_0 x dF_1  (Eqs. 2.5/2.6)
+                cross_set(c0, c1, n2);
+                if (n == 0) fetch(buf, 1, w0, w1);      // record(t) of node 1, under the arithmetic of node 0
+                // D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x delta_k B;  u = gamma J x B;  xi+ = xi + dt u
+                cross_set(n0, dBi, DJ);
+                cross_acc(n1, dBj, DJ);
+                cross_acc(n2, dBk, DJ);
+                cross_set(DJ, Bc[n], uu);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], x[c]);
+                ok = ok && is_finite(x[0] + x[1] + x[2]);
+                if (st[n]) {
+                    T* pn = po + n * a.pitch;
+                    pn[0] = x[0];
+                    pn[a.comp] = x[1];
+                    pn[2 * a.comp] = x[2];
+                }
+            }
+            po += a.plane;
+            tmem::fence_before_sync();
+            ptx::named_arrive(BAR_FREE + buf, NTH);     // the B plane t and record(t) may be overwritten
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                Bm[0][c] = Bc[0][c]; Bm[1][c] = Bc[1][c];
+                Bc[0][c] = Bp[0][c]; Bc[1][c] = Bp[1][c];
+            }
+            buf = bufn;
+        }
+        if (k1 == nz) {   // the top plane (line-tied) is carried through: its xi sits in record(nz-1)
+#pragma unroll
+            for (int n = 0; n < 2; ++n) {
+                uint32_t w0[CW], w1[CW];
+                fetch(buf, n, w0, w1);
+                tmem::wait_ld(w0);
+                tmem::wait_ld(w1);
+                if (st[n]) {
+                    T* pl = out + (long long)(nz - 1) * a.plane + (long long)(gja + n) * a.pitch + gi;
+                    pl[0] = W32::get(w0 + 6 * W32::N);
+                    pl[a.comp] = W32::get(w0 + 7 * W32::N);
+                    pl[2 * a.comp] = W32::get(w1 + 7 * W32::N);
+                }
+            }
+        }
+    }
+    if (!ok) atomicOr(a.flag, FLAG_NUMERIC);
+    tmem::fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem::dealloc<512>(tm_base_s);
+}
+
+// ----------------------------------------------------------------------------------------------- host side
+
+#ifndef MR_DTY
+#define MR_DTY 16
+#define MR_DR 5
+#define MR_DRB 3
+#define MR_DNB 3
+#endif
+constexpr int kDTY = MR_DTY, kDR = MR_DR, kDRB = MR_DRB, kDNB = MR_DNB;
+
+template <typename T>
+inline cudaError_t duo_set_smem(size_t bytes)
+{
+    return cudaFuncSetAttribute(k_step_duo<T, kDTY, kDR, kDRB, kDNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+inline bool build_duo_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* xi0, void* xi1, void* b, int sm_count,
+                           std::string* why)
+{
+    using Ld = DuoLayout<double, kDTY, kDR, kDRB, kDNB>;
+    using Lf = DuoLayout<float, kDTY, kDR, kDRB, kDNB>;
+    p->usable = false;
+    p->f64 = f64;
+    p->g = g;
+    p->xi[0] = xi0;
+    p->xi[1] = xi1;
+    p->b = b;
+    p->name = f64 ? "duo_tmem_f64" : "duo_tmem_f32";
+    const int bw = f64 ? Ld::BW : Lf::BW;
+    if (!encode_map(&p->map_xi[0], f64, xi0, g, bw, kDTY + 4) || !encode_map(&p->map_xi[1], f64, xi1, g, bw, kDTY + 4) ||
+        !encode_map(&p->map_b, f64, b, g, bw, kDTY + 2)) {
+        *why = "cuTensorMapEncodeTiled failed";
+        return false;
+    }
+    p->tiles_x = (g.nx + Ld::TX - 1) / Ld::TX;
+    p->tiles_y = (g.ny + kDTY - 1) / kDTY;
+    p->smem_bytes = f64 ? Ld::BYTES : Lf::BYTES;
+    cudaError_t e = f64 ? duo_set_smem<double>(p->smem_bytes) : duo_set_smem<float>(p->smem_bytes);
+    if (e != cudaSuccess) {
+        *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
+        return false;
+    }
+    choose_chunks(p->tiles_x * p->tiles_y, g.nz, sm_count, &p->nchunks, &p->chunk_len);
+    p->usable = true;
+    return true;
+}
+
+template <typename T>
+inline cudaError_t launch_duo_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream)
+{
+    using L = DuoLayout<T, kDTY, kDR, kDRB, kDNB>;
+    StreamArgs<T> a;
+    a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
+    a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
+    for (int c = 0; c < 3; ++c) a.twoh[c] = (T)p.g.twoh[c];
+    a.dtg = dtg;
+    a.tiles_x = p.tiles_x;
+    a.ntiles = p.tiles_x * p.tiles_y;
+    a.chunk_len = p.chunk_len;
+    a.flag = flag;
+    const int grid = a.ntiles * p.nchunks;
+    k_step_duo<T, kDTY, kDR, kDRB, kDNB><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
+                                                                                       static_cast<T*>(p.xi[1 - cur]), a);
+    return cudaGetLastError();
+}
+
+}  // namespace mr

@@ -311,6 +311,23 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
                     x0[0][c] = f0[c * CSX];
                     x0[1][c] = f0[c * CSX + BW];
                 }
+#ifdef MR_COPY_ONLY   /* experiment: the data movement alone (TMA ring, barrier per plane, coalesced store), no arithmetic */
+                {
+                    if (k + 2 <= nz - 1) ptx::mbar_wait(bar_x + 8u * (uint32_t)sl2, par2);
+                    ptx::mbar_wait(bar_b + 8u * (uint32_t)slb, parb);
+                    const T* bs = sb + slb * L::SLOTB + ob[0];
+                    if (PLAIN || st0) { po[0] = x0[0][0] + T(1e-30) * bs[0]; po[a.comp] = x0[0][1] + T(1e-30) * bs[CSB]; po[2 * a.comp] = x0[0][2] + T(1e-30) * bs[2 * CSB]; }
+                    if (PLAIN || st1) { po[a.pitch] = x0[1][0] + T(1e-30) * bs[BW]; po[a.comp + a.pitch] = x0[1][1] + T(1e-30) * bs[CSB + BW]; po[2 * a.comp + a.pitch] = x0[1][2] + T(1e-30) * bs[2 * CSB + BW]; }
+                    po += a.plane;
+                    ptx::cta_sync();
+                    if (producer) {
+                        if (k + R <= plast) load_x(k + R, (uint32_t)sl0);
+                        if (k + 1 + RB <= blast) load_b(k + 1 + RB, (uint32_t)slb);
+                    }
+                    advance();
+                    continue;
+                }
+#endif
                 T DJ[2][3];     // D J = sum_q n_q x delta_q B (closed form of Eqs. 2.3-2.7), built up in two parts
                 if (inner_k) {
                     // ---- in-plane part of D J of plane k: n_0 x delta_i B + n_1 x delta_j B ----
