@@ -40,7 +40,7 @@ struct DuoLayout {
     static constexpr int BBW = TX + 2, BBH = TY + 2;
     static constexpr int BCS = BBW * BBH;
     static constexpr int BSLOT = round128(3 * BCS * (int)sizeof(T)) / (int)sizeof(T);
-    static constexpr int NAW = TY / 2, NWARPS = 2 * NAW, NTHREADS = NWARPS * 32;
+    static constexpr int NAW = TY / 2, NWARPS = 2 * NAW + 4, NTHREADS = NWARPS * 32;   // A-, F- and four R-warps
     static constexpr size_t OFF_X = 0;
     static constexpr size_t OFF_B0 = OFF_X + (size_t)R * SLOTX * sizeof(T);
     static constexpr size_t OFF_BB = OFF_B0 + (size_t)RB * SLOTB * sizeof(T);
@@ -76,7 +76,11 @@ __device__ __forceinline__ void duo_push(T (&dF)[3][3], const T* __restrict__ bs
 }
 
 template <typename T, int TY, int R, int RB, int NB>
-__global__ void __launch_bounds__(TY * 32, 1)
+#ifndef MR_DUO_MAXREG
+#define MR_DUO_MAXREG 96
+#endif
+// 20 warps x 32 x 96 registers = 60 K of the SM's 64 K
+__global__ void __maxnreg__(MR_DUO_MAXREG)
 k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, T* __restrict__ out,
            const StreamArgs<T> a)
 {
@@ -101,8 +105,9 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const uint32_t bar_x = ptx::smem_u32(smem + L::OFF_BAR), bar_b = bar_x + 8u * R;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const bool isA = warp < NAW;
-    const int widx = isA ? warp : warp - NAW;       // the A-warp and the F-warp of the same rows share widx
+    constexpr int NAG = NAW + 4;                    // warps of the stage-A group (A-warps and R-warps)
+    const bool isA = warp < NAW, isF = warp >= NAW && warp < 2 * NAW;
+    const int widx = isA ? warp : isF ? warp - NAW : 0;       // the A-warp and the F-warp of the same rows share widx
     const int tile = blockIdx.x % a.ntiles, chunk = blockIdx.x / a.ntiles;
     const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY;
     const int nz = a.nz;
@@ -112,7 +117,7 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int pfirst = max(first_p - 1, 0), plast = min(kend + 1, nz - 1);   // xi planes this item touches
     const int bfirst = first_p, blast = kend;                                // b planes
 
-    const bool producer = tid == (NAW - 1) * 32;
+    const bool producer = tid == (2 * NAW + 3) * 32;
     if (producer) {
         for (int s = 0; s < R + RB; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
         ptx::fence_mbar_init();
@@ -129,8 +134,8 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int oB0 = (2 * widx + 1) * BBW + (lane + 1);      // the pair's node 0 inside a shared B plane
     bool ok = true;
 
-    if (isA) {
-        // =============================================== A-warps ===============================================
+    if (!isF) {
+        // ======================== A-warps (tile pairs) and R-warps (halo-1 ring): stage A ========================
         const T twoh[3] = { a.twoh[0], a.twoh[1], a.twoh[2] };
         auto load_x = [&](int p) {
             const uint32_t s = (uint32_t)((p - pfirst) % R);
@@ -149,51 +154,32 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         };
         if (producer) refill(pfirst + R - 1, bfirst + RB - 1);
         auto wait_x = [&](int p) { const int q = p - pfirst; ptx::mbar_wait(bar_x + 8u * (uint32_t)(q % R), (uint32_t)((q / R) & 1)); };
-        auto wait_b = [&](int p) { const int q = p - bfirst; ptx::mbar_wait(bar_b + 8u * (uint32_t)(q % RB), (uint32_t)((q / RB) & 1)); };
         auto xplane = [&](int p) -> const T* { return sx + ((p - pfirst) % R) * L::SLOTX; };
-        auto bplane = [&](int p) -> const T* { return sb + ((p - bfirst) % RB) * L::SLOTB; };
+        const bool plain = i0 > 0 && i0 + TX <= a.nx - 2 && j0 > 0 && j0 + TY <= a.ny - 2;
+        for (int p = pfirst; p <= min(first_p + 1, plast); ++p) wait_x(p);
+        if (first_p == 0 && plast >= 2) wait_x(2);          // the one-sided difference on the bottom face
 
-        // nodes: 0, 1 = the pair (lane, 2 warp), (lane, 2 warp + 1); 2 = a node of the halo-1 ring (warps 0..2)
-        int ti2, tj2;
-        constexpr int NRINGW = 2 + (TY + 15) / 16;
-        static_assert(NRINGW < NAW, "the last A-warp (TMA producer) carries no ring node");
-        bool ring = warp < NRINGW;
-        if (warp == 0) { ti2 = lane; tj2 = -1; }
-        else if (warp == 1) { ti2 = lane; tj2 = TY; }
-        else {
-            ti2 = (lane >> 3) & 1 ? TX : -1;
-            tj2 = (lane & 7) + 8 * (lane >> 4) + 16 * (warp - 2);
-            if (tj2 >= TY) { ring = false; tj2 = 0; }
-        }
+      if (isA) {
         const int ox0 = (2 * warp + 2) * BW + (lane + L::HXL), ob0 = (2 * warp + 1) * BW + (lane + L::HXL);
-        const int ox2 = (tj2 + 2) * BW + (ti2 + L::HXL), ob2 = (tj2 + 1) * BW + (ti2 + L::HXL), oB2 = (tj2 + 1) * BBW + (ti2 + 1);
-        unsigned edge[3];
-        bool dom[3];
-        {
-            const int gis[3] = { gi, gi, i0 + ti2 }, gjs[3] = { gja, gja + 1, j0 + tj2 };
+        unsigned edge[2];
+        bool dom[2];
 #pragma unroll
-            for (int n = 0; n < 3; ++n) {
-                dom[n] = gis[n] >= 0 && gis[n] < a.nx && gjs[n] >= 0 && gjs[n] < a.ny && (n < 2 || ring);
-                edge[n] = !dom[n] ? 0u
-                    : (gis[n] == 0 ? 1u : 0u) | (gis[n] == a.nx - 1 ? 2u : 0u) | (gjs[n] == 0 ? 4u : 0u) | (gjs[n] == a.ny - 1 ? 8u : 0u);
-            }
+        for (int n = 0; n < 2; ++n) {
+            const int gj = gja + n;
+            dom[n] = gi < a.nx && gj < a.ny;
+            edge[n] = !dom[n] ? 0u : (gi == 0 ? 1u : 0u) | (gi == a.nx - 1 ? 2u : 0u) | (gj == 0 ? 4u : 0u) | (gj == a.ny - 1 ? 8u : 0u);
         }
         const bool in_x = gi > 0 && gi < a.nx - 1;
         const bool in_xy[2] = { in_x && gja > 0 && gja < a.ny - 1, in_x && gja + 1 < a.ny - 1 };
-        const bool plain = i0 > 0 && i0 + TX <= a.nx - 2 && j0 > 0 && j0 + TY <= a.ny - 2;
-
-        for (int p = pfirst; p <= min(first_p + 1, plast); ++p) wait_x(p);
-        if (first_p == 0 && plast >= 2) wait_x(2);          // the one-sided difference on the bottom face
-        T xc[2][3], xr[3];                                  // own xi(p-1) of the pair and of the ring node
+        T xc[2][3];                                         // own xi(p-1) of the pair
 #pragma unroll
-        for (int c = 0; c < 3; ++c) { xc[0][c] = T(0); xc[1][c] = T(0); xr[c] = T(0); }
+        for (int c = 0; c < 3; ++c) { xc[0][c] = T(0); xc[1][c] = T(0); }
         if (first_p > 0) {
             const T* f = xplane(first_p - 1);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 xc[0][c] = f[ox0 + c * CSX];
                 xc[1][c] = f[ox0 + c * CSX + BW];
-                xr[c] = f[ox2 + c * CSX];
             }
         }
         auto runA = [&](auto plain_c) {
@@ -282,51 +268,13 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                     if constexpr (CW == 16) { tmem::st16(rec_addr(buf, n, 0), w0); tmem::st16(rec_addr(buf, n, 1), w1); }
                     else { tmem::st8(rec_addr(buf, n, 0), w0); tmem::st8(rec_addr(buf, n, 1), w1); }
                 }
-                if (ring && p >= k0 && p < kend) {
-                    // stage A at the ring node (planes k0 .. kend-1: the planes whose in-plane differences are taken)
-                    T dFr[3][3], nr[3], B[3], inv, xr1[3];
-                    const T* fr = f1 + ox2;
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        xr1[c] = fr[c * CSX];
-                        dFr[c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
-                        dFr[c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
-                    }
-                    if (p == 0) {
-                        const T* f3 = sx + s2 * L::SLOTX;
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) dFr[c][2] = T(4) * f2[ox2 + c * CSX] - T(3) * xr1[c] - f3[ox2 + c * CSX];
-                    } else if (p + 1 <= nz - 1) {
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) dFr[c][2] = f2[ox2 + c * CSX] - xr[c];
-                    } else {
-                        const T* fm = sx + sm2 * L::SLOTX;
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) dFr[c][2] = T(3) * xr1[c] - T(4) * xr[c] + fm[ox2 + c * CSX];
-                    }
-                    if (!PLAIN && edge[2]) face_fix<T, BW, CSX>(fr, edge[2], dFr);
-                    duo_push<T, CSB>(dFr, bs + ob2, twoh, nr, B, inv, ok, PLAIN || dom[2]);
-                    T* d = Bd + oB2;
-                    d[0] = B[0];
-                    d[BCS] = B[1];
-                    d[2 * BCS] = B[2];
-                }
-                if (ring) {
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) xr[c] = f1[ox2 + c * CSX];
-                }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) { xc[0][c] = x1[0][c]; xc[1][c] = x1[1][c]; }
                 tmem::wait_st();
                 tmem::fence_before_sync();
                 ptx::named_arrive(BAR_FULL + buf, NTH);           // B(p) and record(p) are published
-                // every A-warp is done with the xi / b planes p: only the producer's warp waits for the others
-                if (warp == NAW - 1) {
-                    ptx::named_sync(BAR_A + buf, NAW * 32);
-                    if (producer) refill(p + R, p + RB);   // the slots of the planes <= p take the planes up to p + R / p + RB
-                } else {
-                    ptx::named_arrive(BAR_A + buf, NAW * 32);
-                }
+                // this warp is done with the xi / b planes p (the producer's warp collects the arrivals)
+                ptx::named_arrive(BAR_A + buf, NAG * 32);
                 if (++buf == NB) buf = 0;
                 sm2 = sm1; sm1 = s0; s0 = s1; s1 = s2;
                 if (s1 == 0) par1 ^= 1u;                          // the slot of the plane p+1 wrapped around
@@ -336,6 +284,106 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         };
         if (plain) runA(std::true_type{});
         else runA(std::false_type{});
+      } else {
+        // ---- R-warps: warp 2 NAW owns the ring rows j = -1 and j = TY (two nodes per thread), warp 2 NAW + 1 the ring
+        // columns i = -1 and i = TX (8 rows left and 8 rows right per half-warp: distinct banks) and the TMA producer
+        // R-warps: 2 NAW -> ring row j = -1, 2 NAW + 1 -> ring row j = TY, 2 NAW + 2 -> both ring columns,
+        // 2 NAW + 3 -> no node: its lane 0 is the TMA producer and its warp collects the slot-release arrivals
+        const int rw = warp - 2 * NAW;
+        const bool rows = rw < 3;                            // "this warp only arrives on the slot-release barrier"
+        const int nr = rw < 3 ? 1 : 0;
+        int ti[2], tj[2], oxr[2], obr[2], oBr[2];
+        unsigned edge[2];
+        bool dom[2];
+        if (rw == 0) { ti[0] = lane; tj[0] = -1; }
+        else if (rw == 1) { ti[0] = lane; tj[0] = TY; }
+        else { ti[0] = (lane >> 3) & 1 ? TX : -1; tj[0] = (lane & 7) + 8 * (lane >> 4); }
+        ti[1] = ti[0]; tj[1] = tj[0];
+#pragma unroll
+        for (int m = 0; m < 2; ++m) {
+            const int gi2 = i0 + ti[m], gj2 = j0 + tj[m];
+            oxr[m] = (tj[m] + 2) * BW + (ti[m] + L::HXL);
+            obr[m] = (tj[m] + 1) * BW + (ti[m] + L::HXL);
+            oBr[m] = (tj[m] + 1) * BBW + (ti[m] + 1);
+            dom[m] = gi2 >= 0 && gi2 < a.nx && gj2 >= 0 && gj2 < a.ny && tj[m] < TY + 1 && m < nr;
+            edge[m] = !dom[m] ? 0u : (gi2 == 0 ? 1u : 0u) | (gi2 == a.nx - 1 ? 2u : 0u) | (gj2 == 0 ? 4u : 0u) | (gj2 == a.ny - 1 ? 8u : 0u);
+        }
+        T xr[2][3];                                         // own xi(p-1) of the ring nodes
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { xr[0][c] = T(0); xr[1][c] = T(0); }
+        if (first_p > 0) {
+            const T* f = xplane(first_p - 1);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { xr[0][c] = f[oxr[0] + c * CSX]; xr[1][c] = f[oxr[1] + c * CSX]; }
+        }
+        int buf = first_p % NB;
+        int s0 = (first_p - pfirst) % R, s1 = (s0 + 1) % R, s2 = (s0 + 2) % R, sm1 = (s0 + R - 1) % R, sm2 = (s0 + R - 2) % R;
+        uint32_t par1 = (uint32_t)(((first_p + 1 - pfirst) / R) & 1);
+        int sb0 = 0;
+        uint32_t parb = 0u;
+#pragma unroll 1
+        for (int p = first_p; p <= kend; ++p) {
+            const T* f1 = sx + s0 * L::SLOTX;
+            const T* f2 = sx + s1 * L::SLOTX;
+            if (p + 1 <= plast) ptx::mbar_wait(bar_x + 8u * (uint32_t)s1, par1);
+            ptx::mbar_wait(bar_b + 8u * (uint32_t)sb0, parb);
+            const T* bs = sb + sb0 * L::SLOTB;
+            const bool work = p >= k0 && p < kend;              // the planes whose in-plane differences are taken
+            T dFr[2][3][3], x1[2][3];
+#pragma unroll
+            for (int m = 0; m < 2; ++m) {
+                const T* fr = f1 + oxr[m];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    x1[m][c] = fr[c * CSX];
+                    dFr[m][c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
+                    dFr[m][c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
+                }
+                if (p == 0) {
+                    const T* f3 = sx + s2 * L::SLOTX;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) dFr[m][c][2] = T(4) * f2[oxr[m] + c * CSX] - T(3) * x1[m][c] - f3[oxr[m] + c * CSX];
+                } else if (p + 1 <= nz - 1) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) dFr[m][c][2] = f2[oxr[m] + c * CSX] - xr[m][c];
+                } else {
+                    const T* fm = sx + sm2 * L::SLOTX;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) dFr[m][c][2] = T(3) * x1[m][c] - T(4) * xr[m][c] + fm[oxr[m] + c * CSX];
+                }
+                if (edge[m]) face_fix<T, BW, CSX>(fr, edge[m], dFr[m]);
+            }
+            if (p >= first_p + NB) ptx::named_sync(BAR_FREE + buf, NTH);
+            if (work) {
+                T* Bd = sB + buf * L::BSLOT;
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                    if (m < nr) {
+                        T n0[3], B[3], inv;
+                        duo_push<T, CSB>(dFr[m], bs + obr[m], twoh, n0, B, inv, ok, dom[m]);
+                        T* d = Bd + oBr[m];
+                        d[0] = B[0];
+                        d[BCS] = B[1];
+                        d[2 * BCS] = B[2];
+                    }
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { xr[0][c] = x1[0][c]; xr[1][c] = x1[1][c]; }
+            ptx::named_arrive(BAR_FULL + buf, NTH);
+            if (rows) {
+                ptx::named_arrive(BAR_A + buf, NAG * 32);
+            } else {
+                ptx::named_sync(BAR_A + buf, NAG * 32);         // every A- and R-warp is done with the xi / b planes p
+                if (producer) refill(p + R, p + RB);            // the slots of the planes <= p take the planes up to p+R / p+RB
+            }
+            if (++buf == NB) buf = 0;
+            sm2 = sm1; sm1 = s0; s0 = s1; s1 = s2;
+            if (s1 == 0) par1 ^= 1u;
+            if (++s2 == R) s2 = 0;
+            if (++sb0 == RB) { sb0 = 0; parb ^= 1u; }
+        }
+      }
     } else {
         // =============================================== F-warps ===============================================
         auto ownB = [&](int buf, T(&B)[2][3]) {

@@ -167,6 +167,10 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
     tj[0] = 2 * warp;
     tj[1] = 2 * warp + 1;
     bool ring = false;
+#ifdef MR_NO_RING
+    if (true) { ti[2] = 0; tj[2] = 0; }
+    else
+#endif
     if (warp == 0) { ring = true; ti[2] = lane; tj[2] = -1; }
     else if (warp == 1) { ring = true; ti[2] = lane; tj[2] = TY; }
     else if (warp < 4) {
@@ -303,7 +307,11 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
                 T(&Bn)[2][3] = Bq[u ^ 1];
                 T(&x1)[2][3] = Xq[u];
                 T(&x2)[2][3] = Xq[u ^ 1];
+#ifdef MR_NO_STAGEB
+                const bool inner_k = false;
+#else
                 const bool inner_k = k > 0;          // (k <= nz-2 inside this loop)
+#endif
                 const T* f0 = sx + sl0 * L::SLOTX + ox[0];
                 T x0[2][3];                           // own xi of plane k (re-read: plane k stays in its slot)
 #pragma unroll
@@ -352,7 +360,9 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
                     T dF[2][3][3];
                     const T* f = sx + sl1 * L::SLOTX + ox[0];
                     if (k + 2 <= nz - 1) {
+#ifndef MR_NO_REFILL
                         ptx::mbar_wait(bar_x + 8u * (uint32_t)sl2, par2);
+#endif
                         const T* f2 = sx + sl2 * L::SLOTX + ox[0];
 #pragma unroll
                         for (int c = 0; c < 3; ++c) {
@@ -381,7 +391,9 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
                         if (edge[0]) face_fix<T, BW, CSX>(f, edge[0], dF[0]);
                         if (edge[1]) face_fix<T, BW, CSX>(f + BW, edge[1], dF[1]);
                     }
+#ifndef MR_NO_REFILL
                     ptx::mbar_wait(bar_b + 8u * (uint32_t)slb, parb);
+#endif
                     const T* bs = sb + slb * L::SLOTB + ob[0];
                     push_forward_n<T, CSB>(dF[0], bs, twoh, nnew[0], Bn[0], invq[u ^ 1][0], ok, PLAIN || dom[0]);
                     push_forward_n<T, CSB>(dF[1], bs + BW, twoh, nnew[1], Bn[1], invq[u ^ 1][1], ok, PLAIN || dom[1]);
@@ -440,9 +452,15 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
                     po[2 * a.comp + a.pitch] = x0[1][2];
                 }
                 po += a.plane;
+#ifndef MR_NO_BAR
                 ptx::cta_sync();
+#endif
                 // the xi plane k and the b plane k+1 are dead now: their slots take the planes k+R and k+1+RB
+#ifdef MR_NO_REFILL
+                if (false) {
+#else
                 if (producer) {
+#endif
                     if (k + R <= plast) load_x(k + R, (uint32_t)sl0);
                     if (k + 1 + RB <= blast) load_b(k + 1 + RB, (uint32_t)slb);
                 }
@@ -458,7 +476,9 @@ k_step_pair(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
         if (st0) { pl[0] = pt[0]; pl[a.comp] = pt[CSX]; pl[2 * a.comp] = pt[2 * CSX]; }
         if (st1) { pl[a.pitch] = pt[BW]; pl[a.comp + a.pitch] = pt[CSX + BW]; pl[2 * a.comp + a.pitch] = pt[2 * CSX + BW]; }
     }
+#ifndef MR_NO_FLAG
     if (!ok) atomicOr(a.flag, FLAG_NUMERIC);
+#endif
 }
 
 // ----------------------------------------------------------------------------------------------- host side
