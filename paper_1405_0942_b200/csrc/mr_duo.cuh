@@ -331,7 +331,7 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             const bool work = p >= k0 && p < kend;              // the planes whose in-plane differences are taken
             T dFr[2][3][3], x1[2][3];
 #pragma unroll
-            for (int m = 0; m < 2; ++m) {
+            for (int m = 0; m < 1; ++m) {
                 const T* fr = f1 + oxr[m];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -357,7 +357,7 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             if (work) {
                 T* Bd = sB + buf * L::BSLOT;
 #pragma unroll
-                for (int m = 0; m < 2; ++m) {
+                for (int m = 0; m < 1; ++m) {
                     if (m < nr) {
                         T n0[3], B[3], inv;
                         duo_push<T, CSB>(dFr[m], bs + obr[m], twoh, n0, B, inv, ok, dom[m]);
@@ -369,7 +369,7 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 }
             }
 #pragma unroll
-            for (int c = 0; c < 3; ++c) { xr[0][c] = x1[0][c]; xr[1][c] = x1[1][c]; }
+            for (int c = 0; c < 3; ++c) xr[0][c] = x1[0][c];
             ptx::named_arrive(BAR_FULL + buf, NTH);
             if (rows) {
                 ptx::named_arrive(BAR_A + buf, NAG * 32);
