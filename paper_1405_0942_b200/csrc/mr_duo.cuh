@@ -70,9 +70,10 @@ __device__ __forceinline__ void duo_push(T (&dF)[3][3], const T* __restrict__ bs
     const T D = dF[0][0] * n0[0] + dF[1][0] * n0[1] + dF[2][0] * n0[2];
     ok = ok && (positive_finite(D) || !in_dom);
     inv = fast_rcp(D);
-    const T b0 = bs[0] * inv, b1 = bs[CSB] * inv, b2 = bs[2 * CSB] * inv;
+    // dF b first, the division last: the nine products do not wait for the reciprocal's Newton chain
+    const T b0 = bs[0], b1 = bs[CSB], b2 = bs[2 * CSB];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) B[c] = dF[c][0] * b0 + dF[c][1] * b1 + dF[c][2] * b2;
+    for (int c = 0; c < 3; ++c) B[c] = (dF[c][0] * b0 + dF[c][1] * b1 + dF[c][2] * b2) * inv;
 }
 
 template <typename T, int TY, int R, int RB, int NB>
