@@ -269,7 +269,13 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     const T* b = static_cast<const T*>(c->b());
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     const int threads = c->grid.nx >= 256 ? 256 : (c->grid.nx >= 128 ? 128 : (c->grid.nx >= 64 ? 64 : 32));
-    if (op == MR_OP_MIMETIC)
+    const bool fused = op == MR_OP_MIMETIC && c->plan5.usable && (c->force_variant == 0 || c->force_variant == 6) &&
+                       c->plan5.tiles_x * c->plan5.tiles_y * c->plan5.nchunks <= kMaxPartialBlocks;
+    if (fused) {
+        // the streaming pass of the step kernel with the update replaced by the reduction (mr_duo.cuh, DIAG)
+        cudaError_t e = launch_duo_diag<T>(c->plan5, c->cur, c->partials(), &blocks, c->flag(), c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, "streaming diagnostics launch", e);
+    } else if (op == MR_OP_MIMETIC)
         k_diag<T, 0><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());
     else
         k_diag<T, 1><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());

@@ -20,6 +20,7 @@
 #pragma once
 #include <type_traits>
 
+#include "mr_generic.cuh"
 #include "mr_pair.cuh"
 #include "mr_tmem.cuh"
 
@@ -76,7 +77,7 @@ __device__ __forceinline__ void duo_push(T (&dF)[3][3], const T* __restrict__ bs
     for (int c = 0; c < 3; ++c) B[c] = (dF[c][0] * b0 + dF[c][1] * b1 + dF[c][2] * b2) * inv;
 }
 
-template <typename T, int TY, int R, int RB, int NB>
+template <typename T, int TY, int R, int RB, int NB, bool DIAG>
 #ifndef MR_DUO_MAXREG
 #define MR_DUO_MAXREG 96
 #endif
@@ -134,6 +135,7 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const bool st[2] = { gi < a.nx && gja < a.ny, gi < a.nx && gja + 1 < a.ny };
     const int oB0 = (2 * widx + 1) * BBW + (lane + 1);      // the pair's node 0 inside a shared B plane
     bool ok = true;
+    DiagPartial diag_acc = { 0.0, 0.0, 0.0, INFINITY };   // DIAG: the F-warp's partial (valid in lane 0)
 
     if (!isF) {
         // ======================== A-warps (tile pairs) and R-warps (halo-1 ring): stage A ========================
@@ -400,6 +402,27 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             else { tmem::ld8(rec_addr(buf, n, 0), w0); tmem::ld8(rec_addr(buf, n, 1), w1); }
         };
         T Bm[2][3], Bc[2][3];                           // own B(t-1), B(t) of the pair
+        // DIAG: the same pass with the update replaced by the reduction of S6 (E, max |JxB|, max |JxB|/B^2, min D)
+        DiagPartial acc = { 0.0, 0.0, 0.0, INFINITY };
+        const bool f_in_x = gi > 0 && gi < a.nx - 1;
+        const bool f_in_xy[2] = { f_in_x && gja > 0 && gja < a.ny - 1, f_in_x && gja + 1 < a.ny - 1 };
+        double zxy[2];                                  // trapezoid weights of the node's column (Eq. 3.13)
+#pragma unroll
+        for (int n = 0; n < 2; ++n)
+            zxy[n] = ((gi == 0 || gi == a.nx - 1) ? 0.5 : 1.0) * ((gja + n == 0 || gja + n == a.ny - 1) ? 0.5 : 1.0);
+        auto diag_node = [&](int n, int k, const T(&c0)[3], const T(&n0)[3], const T(&B)[3], const T(&uu)[3]) {
+            if (!st[n]) return;
+            const double D = (double)c0[0] * n0[0] + (double)c0[1] * n0[1] + (double)c0[2] * n0[2];
+            const double b2 = (double)B[0] * B[0] + (double)B[1] * B[1] + (double)B[2] * B[2];
+            const bool kface = k == 0 || k == nz - 1;
+            DiagPartial v = { zxy[n] * (kface ? 0.5 : 1.0) * b2 * D, 0.0, 0.0, D };
+            if (f_in_xy[n] && !kface) {
+                const double fm = sqrt((double)uu[0] * uu[0] + (double)uu[1] * uu[1] + (double)uu[2] * uu[2]) / D;
+                v.fmax = fm;
+                v.xi = fm / b2;
+            }
+            diag_combine(acc, v);
+        };
 #pragma unroll
         for (int c = 0; c < 3; ++c) { Bm[0][c] = T(0); Bm[1][c] = T(0); }
         int buf = first_p % NB;                         // buffer of the plane t
@@ -455,14 +478,18 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 cross_acc(n1, dBj, DJ);
                 cross_acc(n2, dBk, DJ);
                 cross_set(DJ, Bc[n], uu);
+                if constexpr (DIAG) {
+                    diag_node(n, t, c0, n0, Bc[n], uu);
+                } else {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], x[c]);
-                ok = ok && is_finite(x[0] + x[1] + x[2]);
-                if (st[n]) {
-                    T* pn = po + n * a.pitch;
-                    pn[0] = x[0];
-                    pn[a.comp] = x[1];
-                    pn[2 * a.comp] = x[2];
+                    for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], x[c]);
+                    ok = ok && is_finite(x[0] + x[1] + x[2]);
+                    if (st[n]) {
+                        T* pn = po + n * a.pitch;
+                        pn[0] = x[0];
+                        pn[a.comp] = x[1];
+                        pn[2 * a.comp] = x[2];
+                    }
                 }
             }
             po += a.plane;
@@ -482,7 +509,16 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 fetch(buf, n, w0, w1);
                 tmem::wait_ld(w0);
                 tmem::wait_ld(w1);
-                if (st[n]) {
+                if constexpr (DIAG) {
+                    T c0[3], n0[3];
+                    const T zero[3] = { T(0), T(0), T(0) };
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        c0[c] = W32::get(w0 + c * W32::N);
+                        n0[c] = W32::get(w1 + (3 + c) * W32::N);
+                    }
+                    diag_node(n, nz - 1, c0, n0, Bc[n], zero);
+                } else if (st[n]) {
                     T* pl = out + (long long)(nz - 1) * a.plane + (long long)(gja + n) * a.pitch + gi;
                     pl[0] = W32::get(w0 + 6 * W32::N);
                     pl[a.comp] = W32::get(w0 + 7 * W32::N);
@@ -490,10 +526,33 @@ k_step_duo(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 }
             }
         }
+        if constexpr (DIAG) {
+            // fixed-order reduction: lanes by a shuffle tree, then the F-warps in index order (below)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                DiagPartial w;
+                w.e = __shfl_down_sync(0xffffffffu, acc.e, o);
+                w.fmax = __shfl_down_sync(0xffffffffu, acc.fmax, o);
+                w.xi = __shfl_down_sync(0xffffffffu, acc.xi, o);
+                w.dmin = __shfl_down_sync(0xffffffffu, acc.dmin, o);
+                diag_combine(acc, w);
+            }
+            diag_acc = acc;
+        }
     }
     if (!ok) atomicOr(a.flag, FLAG_NUMERIC);
     tmem::fence_before_sync();
-    __syncthreads();
+    __syncthreads();                                    // the pipeline is drained: shared memory is free
+    if constexpr (DIAG) {
+        DiagPartial* sh = reinterpret_cast<DiagPartial*>(smem);
+        if (isF && lane == 0) sh[widx] = diag_acc;
+        __syncthreads();
+        if (tid == 0) {
+            DiagPartial v = sh[0];
+            for (int w = 1; w < NAW; ++w) diag_combine(v, sh[w]);
+            reinterpret_cast<DiagPartial*>(out)[blockIdx.x] = v;
+        }
+    }
     if (warp == 0) tmem::dealloc<512>(tm_base_s);
 }
 
@@ -510,7 +569,9 @@ constexpr int kDTY = MR_DTY, kDR = MR_DR, kDRB = MR_DRB, kDNB = MR_DNB;
 template <typename T>
 inline cudaError_t duo_set_smem(size_t bytes)
 {
-    return cudaFuncSetAttribute(k_step_duo<T, kDTY, kDR, kDRB, kDNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    cudaError_t e = cudaFuncSetAttribute(k_step_duo<T, kDTY, kDR, kDRB, kDNB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_step_duo<T, kDTY, kDR, kDRB, kDNB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
 inline bool build_duo_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* xi0, void* xi1, void* b, int sm_count,
@@ -558,8 +619,29 @@ inline cudaError_t launch_duo_step(const StreamPlan& p, int cur, T dtg, int* fla
     a.chunk_len = p.chunk_len;
     a.flag = flag;
     const int grid = a.ntiles * p.nchunks;
-    k_step_duo<T, kDTY, kDR, kDRB, kDNB><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
-                                                                                       static_cast<T*>(p.xi[1 - cur]), a);
+    k_step_duo<T, kDTY, kDR, kDRB, kDNB, false><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
+                                                                                              static_cast<T*>(p.xi[1 - cur]), a);
+    return cudaGetLastError();
+}
+
+// S6 of the state in buffer `cur` by the same pass (no update, no store): one DiagPartial per CTA into `partials`
+template <typename T>
+inline cudaError_t launch_duo_diag(const StreamPlan& p, int cur, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
+{
+    using L = DuoLayout<T, kDTY, kDR, kDRB, kDNB>;
+    StreamArgs<T> a;
+    a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
+    a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
+    for (int c = 0; c < 3; ++c) a.twoh[c] = (T)p.g.twoh[c];
+    a.dtg = (T)0;
+    a.tiles_x = p.tiles_x;
+    a.ntiles = p.tiles_x * p.tiles_y;
+    a.chunk_len = p.chunk_len;
+    a.flag = flag;
+    const int grid = a.ntiles * p.nchunks;
+    *nblocks = grid;
+    k_step_duo<T, kDTY, kDR, kDRB, kDNB, true><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
+                                                                                             reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();
 }
 
