@@ -97,7 +97,7 @@ mr_status mr_set_B0(mr_ctx* ctx, const void* B0_dev);
 mr_status mr_set_B0_host(mr_ctx* ctx, const void* B0_host);
 
 /* Set the node positions x (dense, context dtype), e.g. a displaced initial grid or a checkpoint; resets
- * time/steps and clears a numeric failure.  Line-tied boundary nodes must equal X (|x - X| <= 1e-6*h),
+ * time/steps and clears a numeric failure.  Line-tied boundary nodes must equal X (|x - X| <= 1e-6*h, plus 2.4e-7*|X| of input rounding when the context is fp32),
  * otherwise MR_ERR_INVALID_ARG is returned and the state is unchanged.  (Synchronises for that check.) */
 mr_status mr_set_x(mr_ctx* ctx, const void* x_dev);
 mr_status mr_set_x_host(mr_ctx* ctx, const void* x_host);

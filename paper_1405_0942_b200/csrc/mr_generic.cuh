@@ -42,7 +42,9 @@ __global__ void k_import_x(const T* __restrict__ x, T* __restrict__ xi, GridP<T>
         const double X = ref_coord(d.lo[c], d.h[c], idx[c]);
         double v = (double)x[c * N + q] - X;
         if (bnd) {
-            if (!(fabs(v) <= 1e-6 * d.h[c])) off = true;
+            // on the reference grid up to 1e-6 h, plus the rounding of X itself when x comes in as fp32
+            const double tol = 1e-6 * d.h[c] + (sizeof(T) == 4 ? 2.4e-7 * fabs(X) : 0.0);
+            if (!(fabs(v) <= tol)) off = true;
             v = 0.0;
         }
         xi[c * g.comp + p] = (T)v;

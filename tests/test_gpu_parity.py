@@ -304,3 +304,19 @@ def test_full_size_config4_one_step_matches_oracle(mr):
     o = mro.diagnostics(g.n, g.lo, g.hi, x0, B0)
     for k in ("energy", "max_jxb", "xi", "min_det"):
         assert d[k] == pytest.approx(o[k], rel=TOL_STEP), k
+
+
+def test_fp32_context_accepts_the_fp32_rounding_of_the_reference_grid(mr):
+    """mr_set_x on an fp32 context: boundary nodes given as float32(X) are on the reference grid (|X|/h is large
+    on config 5: 4 / (8/511)), one really displaced boundary node is still refused."""
+    g = I.Grid((64, 64, 64), (-4.0, -4.0, -4.0), (4.0, 4.0, 4.0))
+    X = I.reference_grid(g)
+    B0 = I.twist_field(g, (I.Twist(1.0, 1.0, 0.0, 0.0),))
+    sim = mr.Relaxation(g.n, g.lo, g.hi, dtype="f32")
+    sim.set_B0(dev(B0, torch.float32))
+    sim.set_x(dev(X, torch.float32))
+    sim.step(2, 0.25 * I.stable_dt(B0, g))
+    bad = X.copy()
+    bad[0, 0, 5, 5] += 1e-3 * g.h[0]
+    with pytest.raises(mr.MrError):
+        sim.set_x(dev(bad, torch.float32))
