@@ -487,6 +487,9 @@ inline PFN_encodeTiled get_encode_fn()
 constexpr int kTX = 32, kTY = 16, kR = 6, kRB = 3;
 constexpr bool kKEEPX = false;
 
+#ifndef MR_L2_PROMOTION
+#define MR_L2_PROMOTION CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+#endif
 inline bool encode_map(CUtensorMap* m, bool f64, void* base, const StreamGeom& g, int bw, int bh)
 {
     PFN_encodeTiled enc = get_encode_fn();
@@ -497,7 +500,7 @@ inline bool encode_map(CUtensorMap* m, bool f64, void* base, const StreamGeom& g
     cuuint32_t box[4] = { (cuuint32_t)bw, (cuuint32_t)bh, 1, 3 };
     cuuint32_t estr[4] = { 1, 1, 1, 1 };
     CUresult r = enc(m, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, MR_L2_PROMOTION,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
 }
