@@ -31,6 +31,11 @@ if ROOT not in sys.path:
 METRIC = "grid-point updates/s (fp64, mimetic curl)"
 UNIT = "updates/s"
 BYTES_PER_UPDATE = {"f64": 72.0, "f32": 36.0}   # read xi 3T + read b 3T + write xi' 3T
+# direct operator (--operator direct): bound by plain FP64 arithmetic, not HBM.  FLOPs per update counted
+# in the SASS of k_step_generic<double,1> (134 DFMA x 2 + 108 DADD + 86 DMUL); peak = 148 SMs x 64 FP64 lanes x
+# 2 FLOP x 1.965 GHz (B200_PROFILING.md unit counts and clocks)
+DIRECT_FLOP_PER_UPDATE = 462.0
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 
 # ---------------------------------------------------------------------------------------------- helpers (CPU)
@@ -235,13 +240,14 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident throughput: W warm-up steps, then ONE timed mr_step(K) ----
-    sim.step(max(args.warmup, 3), dt)
+    op = args.operator
+    sim.step(max(args.warmup, 3), dt, op)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     with ClockSampler(local_rank) as clocks:
         l0 = sim.launch_count
         e0.record()
-        sim.step(args.steps, dt)
+        sim.step(args.steps, dt, op)
         e1.record()
         barrier()
         launches = sim.launch_count - l0
@@ -249,7 +255,7 @@ def run_ours(args):
     variant = sim.step_variant
     ms_all, updates_all = aggregate_over_ranks(ms, nodes * args.steps, dist if world > 1 else None)
     value = updates_all / (ms_all * 1e-3)
-    diag = sim.diagnostics()
+    diag = sim.diagnostics(op)
 
     # ---- roofline of the dominant (only) kernel: algorithmic bytes per launch / average launch duration ----
     peak, peak_src = measured_peak_gbs()
@@ -258,19 +264,24 @@ def run_ours(args):
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": recorded_traffic(cfg.name, variant), "peak_source": peak_src, "kernel": variant,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE[dtype] * nodes, "launch_ms": launch_ms}
+    if op == "direct":
+        tf = DIRECT_FLOP_PER_UPDATE * nodes / (launch_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
+                    "traffic": None, "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 x 1.965 GHz", "kernel": variant,
+                    "algorithmic_flop_per_launch": DIRECT_FLOP_PER_UPDATE * nodes, "launch_ms": launch_ms}
 
     # ---- end to end through the host-buffer entry points: H2D of x, one step, D2H of x, every step ----
     xh = torch.from_numpy(x0).to(td).pin_memory()
     oh = torch.empty_like(xh).pin_memory()
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     sim.set_x(xh)
-    sim.step(1, dt)
+    sim.step(1, dt, op)
     sim.get_fields_into(x=oh)
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         sim.set_x(xh)                 # mr_set_x_host: pinned host -> device (+ layout import)
-        sim.step(1, dt)               # mr_step
+        sim.step(1, dt, op)           # mr_step
         sim.get_fields_into(x=oh)     # mr_get_fields_host: device -> pinned host
         xh, oh = oh, xh
     barrier()
@@ -288,10 +299,10 @@ def run_ours(args):
 
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "metric": METRIC if op == "mimetic" else METRIC.replace("mimetic", "direct"), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": dtype, "data": "synthetic",
-            "config": {"workload": "%s %dx%dx%d %s mimetic, line-tied, forward Euler dt=%.3e" % ((cfg.name,) + g.n + ("fp64" if dtype == "f64" else "fp32", dt)),
+            "config": {"workload": "%s %dx%dx%d %s %s, line-tied, forward Euler dt=%.3e" % ((cfg.name,) + g.n + ("fp64" if dtype == "f64" else "fp32", op, dt)),
                        "nodes": nodes, "l2_policy": "working set %.2f GB >> 126 MB L2 (no flush needed)" % (3 * fbytes / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "kernel": variant},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
@@ -313,6 +324,7 @@ def main(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5"])
     ap.add_argument("--variant", default="auto", choices=["auto", "generic", "stream", "pair", "lean", "park", "duo"])
+    ap.add_argument("--operator", default="mimetic", choices=["mimetic", "direct"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)
