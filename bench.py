@@ -32,9 +32,9 @@ METRIC = "grid-point updates/s (fp64, mimetic curl)"
 UNIT = "updates/s"
 BYTES_PER_UPDATE = {"f64": 72.0, "f32": 36.0}   # read xi 3T + read b 3T + write xi' 3T
 # direct operator (--operator direct): bound by plain FP64 arithmetic, not HBM.  FLOPs per update counted
-# in the SASS of k_step_generic<double,1> (134 DFMA x 2 + 108 DADD + 86 DMUL); peak = 148 SMs x 64 FP64 lanes x
+# in the SASS of k_step_direct<double> (116 DFMA x 2 + 90 DADD + 68 DMUL); peak = 148 SMs x 64 FP64 lanes x
 # 2 FLOP x 1.965 GHz (B200_PROFILING.md unit counts and clocks)
-DIRECT_FLOP_PER_UPDATE = 462.0
+DIRECT_FLOP_PER_UPDATE = 390.0
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 

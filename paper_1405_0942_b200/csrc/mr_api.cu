@@ -14,6 +14,7 @@
 #include "mr_lean.cuh"
 #include "mr_park.cuh"
 #include "mr_duo.cuh"
+#include "mr_direct.cuh"
 
 using namespace mr;
 
@@ -82,6 +83,7 @@ struct mr_ctx {
     StreamPlan plan3;   // ... for the lean-state streaming kernel (mr_lean.cuh)
     StreamPlan plan4;   // ... for the TMEM-parked streaming kernel (mr_park.cuh)
     StreamPlan plan5;   // ... and for the warp-specialised streaming kernel (mr_duo.cuh)
+    StreamPlan plan6;   // the streaming kernel of the direct-derivative operator (mr_direct.cuh)
     std::string err;
 
     void* xi(int w) const { return ws + L.off_xi[w]; }
@@ -227,13 +229,15 @@ mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
     const bool use_stream = mim && !use_duo && !use_park && !use_lean && !use_pair && (fv == 0 || fv == 2) && c->plan.usable;
     if ((fv == 2 && !use_stream) || (fv == 3 && !use_pair) || (fv == 4 && !use_lean) || (fv == 5 && !use_park) || (fv == 6 && !use_duo))
         return fail(c, MR_ERR_INVALID_ARG, "mr_step: a streaming kernel was forced but does not take this grid/operator");
-    c->variant = use_duo ? c->plan5.name : use_park ? c->plan4.name : use_lean ? c->plan3.name : use_pair ? c->plan2.name : use_stream ? c->plan.name
+    const bool use_dstream = !mim && fv == 0 && c->plan6.usable;
+    c->variant = use_dstream ? c->plan6.name : use_duo ? c->plan5.name : use_park ? c->plan4.name : use_lean ? c->plan3.name : use_pair ? c->plan2.name : use_stream ? c->plan.name
                  : (mim ? "generic_mimetic" : "generic_direct");
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     for (int64_t s = 0; s < n; ++s) {
-        if (use_duo || use_park || use_lean || use_pair || use_stream) {
+        if (use_dstream || use_duo || use_park || use_lean || use_pair || use_stream) {
             const T dtg = (T)(dt * c->gamma);
-            cudaError_t e = use_duo ? launch_duo_step<T>(c->plan5, c->cur, dtg, c->flag(), c->stream)
+            cudaError_t e = use_dstream ? launch_direct_step<T>(c->plan6, c->cur, dtg, c->flag(), c->stream)
+                            : use_duo ? launch_duo_step<T>(c->plan5, c->cur, dtg, c->flag(), c->stream)
                             : use_park ? launch_park_step<T>(c->plan4, c->cur, dtg, c->flag(), c->stream)
                             : use_lean ? launch_lean_step<T>(c->plan3, c->cur, dtg, c->flag(), c->stream)
                             : use_pair ? launch_pair_step<T>(c->plan2, c->cur, dtg, c->flag(), c->stream)
@@ -385,6 +389,10 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     if (!build_duo_plan(&c->plan5, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
         c->plan5.usable = false;
         c->plan5.why = why;
+    }
+    if (!build_direct_plan(&c->plan6, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+        c->plan6.usable = false;
+        c->plan6.why = why;
     }
     *out = c;
     return MR_OK;
