@@ -320,3 +320,38 @@ def test_fp32_context_accepts_the_fp32_rounding_of_the_reference_grid(mr):
     bad[0, 0, 5, 5] += 1e-3 * g.h[0]
     with pytest.raises(mr.MrError):
         sim.set_x(dev(bad, torch.float32))
+
+
+@pytest.mark.parametrize("variant", ["auto", "generic"])
+def test_fp32_direct_operator_within_1e5_of_fp64(mr, variant):
+    """The direct-derivative operator in fp32 (streaming kernel under "auto", global-memory kernel under "generic")
+    against the fp64 GPU run of the same kernel and the fp64 oracle."""
+    cfg = I.scaled(I.CONFIGS["C5"], (64, 64, 64))
+    g = cfg.grid
+    x0, B0, dt = I.make(cfg)
+    s64 = make_sim(mr, g, x0, B0, "f64", variant)
+    s32 = make_sim(mr, g, x0, B0, "f32", variant)
+    s64.step(50, dt, "direct")
+    s32.step(50, dt, "direct")
+    assert s64.step_variant == ("direct_tma_f64" if variant == "auto" else "generic_direct")
+    x64 = s64.get_fields(x=True)["x"].cpu().numpy()
+    x32 = s32.get_fields(x=True)["x"].double().cpu().numpy()
+    assert nrel(x32, x64) < TOL_F32
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 50, op=mro.DIRECT)
+    assert nrel(x64, ref) < TOL_100
+
+
+def test_steps_and_diagnostics_are_deterministic(mr):
+    """Fixed-order reductions and no atomics on the data path: two runs from the same state are bit-identical, for
+    the positions and for the four diagnostics (both operators)."""
+    g, x0, B0, dt = case("wide")
+    outs = []
+    for _ in range(2):
+        sim = make_sim(mr, g, x0, B0)
+        sim.step(7, dt)
+        sim.step(3, dt, "direct")
+        d = sim.diagnostics()
+        outs.append((sim.get_fields(x=True)["x"].cpu().numpy(), d))
+    assert np.array_equal(outs[0][0], outs[1][0])
+    for k in ("energy", "max_jxb", "xi", "min_det"):
+        assert outs[0][1][k] == outs[1][1][k], k
