@@ -1,21 +1,27 @@
 // mr_duo.cuh -- the warp-specialised streaming step kernel for the mimetic operator (S1-S5 in one pass).
 //
-// ncu of the register-paired kernel (profiles/r1c): one CTA of 8 warps per SM, 255 registers, every pipe below 45 %
-// and the warps waiting on each other's latencies -- the kernel is bound by the number of nodes the register file
-// can keep in flight, not by HBM (the same TMA ring with the arithmetic stubbed out runs at 96 % of the measured
-// copy bandwidth).  This kernel splits the work of a node between two warps that hand the node's state over through
-// Tensor Memory (mr_tmem.cuh), so that 16 warps of 128 registers share the SM and the two roles run out of step:
+// ncu of the register-paired kernel (profiles/r1c_full.md): one CTA of 8 warps per SM, 255 registers, every pipe
+// below 45 % and the warps waiting on each other's latencies -- the kernel is bound by the number of nodes the
+// register file can keep in flight, not by HBM (the same TMA ring with the arithmetic stubbed out runs at 96 % of the
+// measured copy bandwidth; the halo-1 ring alone cost 0.14 of its 0.64 ms because it sat on the critical path of half
+// the warps).  This kernel splits the work of a node between warps that hand the node's state over through Tensor
+// Memory (mr_tmem.cuh), so that 20 warps of 96 registers share the SM and the roles run out of step:
 //
-//   A-warps (0..TY/2-1, lane = i, rows 2a and 2a+1; the first ones also carry a node of the halo-1 ring)
-//       plane p:  dF from the xi ring in shared memory (TMA), area vectors n_q (Eqs. 2.5/2.6), D = det dF,
-//                 B(p) = dF b / D (Eq. 2.1) -> shared B plane p % NB;   record(p) = n_0, n_1, n_2, s = dt gamma / D,
-//                 own xi(p) -> TMEM buffer p % NB;   bar.arrive FULL[p % NB]
-//   F-warps (TY/2..TY-1, same lanes and rows: the partner warp sits in the same TMEM lane quarter)
-//       plane t:  bar.sync FULL[(t+1) % NB];  D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x (B(t+1) - B(t-1))
-//                 (closed form of Eqs. 2.3-2.7) from record(t), the shared B plane t and the own B(t-1), B(t), B(t+1);
-//                 u = gamma J x B (Eq. 1.5);  xi+ = xi + dt u -> HBM;   bar.arrive FREE[t % NB]
-// The A-warps wait on FREE[p % NB] before they overwrite a buffer, so they run up to NB-1 planes ahead of the
-// F-warps; the xi / b rings are touched by the A-warps only and recycled behind a barrier of their own.
+//   A-warps (0..TY/2-1, lane = i, rows 2a and 2a+1)
+//       plane p:  dF from the xi ring in shared memory (TMA; the j-differences inside the pair and the k-differences
+//                 from registers), n_0 = dF_1 x dF_2 (area vector, Eqs. 2.5/2.6), D = dF_0 . n_0, 1/D,
+//                 B(p) = dF b / D (Eq. 2.1) -> shared B plane p % NB;   record(p) = dF, n_0, s = dt gamma / D, own xi(p)
+//                 (16 values) -> TMEM buffer p % NB (tcgen05.st);   bar.arrive FULL[p % NB]
+//   R-warps (TY..TY+3: ring row below, ring row above, both ring columns, TMA producer)
+//       plane p:  B(p) of the tile's halo-1 ring, one node per thread -> shared B plane;  bar.arrive FULL[p % NB];
+//                 the producer's warp collects the slot-release arrivals of the A- and R-warps and refills the rings
+//   F-warps (TY/2..TY-1, same lanes and rows as the A-warps: the partner warp sits in the same TMEM lane quarter)
+//       plane t:  record(t) (tcgen05.ld), n_1 = dF_2 x dF_0, n_2 = dF_0 x dF_1;  bar.sync FULL[(t+1) % NB];
+//                 D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x (B(t+1) - B(t-1))  (closed form of Eqs. 2.3-2.7) from
+//                 the shared B plane t and the own B(t-1), B(t), B(t+1);  u = gamma J x B (Eq. 1.5);
+//                 xi+ = xi + dt u -> HBM   (DIAG: the reduction of S6 instead);   bar.arrive FREE[t % NB]
+// The A- and R-warps wait on FREE[p % NB] before they overwrite a buffer, so they run up to NB-1 planes ahead of the
+// F-warps; the xi / b rings are touched by the A- and R-warps only and recycled behind barriers of their own.
 // B, J, u never touch HBM: the algorithmic traffic is read xi + read b + write xi+ = 9 elements per node.
 #pragma once
 #include <type_traits>
