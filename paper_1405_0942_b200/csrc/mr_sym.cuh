@@ -12,13 +12,15 @@
 // (no A/F imbalance), and nobody waits for the slowest warp of the current plane.  A buffer p % NB is overwritten
 // NB planes later; a warp that starts A(p) has seen FULL[p-2] complete, i.e. every warp has finished F(p-4): NB = 4.
 #pragma once
+#include <type_traits>
+
 #include "mr_duo.cuh"
 
 namespace mr {
 
 template <typename T, int TY, int R, int RB, int NB>
 struct SymLayout {
-    static_assert(TY == 16 && R >= 4 && RB >= 2 && NB >= 4, "tile / ring sizes");
+    static_assert(TY == 16 && R >= 4 && RB == R && NB >= 4, "tile / ring sizes (xi and b share the ring positions)");
     static constexpr int TX = 32;
     static constexpr int HXL = 16 / (int)sizeof(T), HXR = 2 * HXL;
     static constexpr int BW = TX + HXL + HXR;
@@ -36,7 +38,7 @@ struct SymLayout {
     static constexpr size_t OFF_B0 = OFF_X + (size_t)R * SLOTX * sizeof(T);
     static constexpr size_t OFF_BB = OFF_B0 + (size_t)RB * SLOTB * sizeof(T);
     static constexpr size_t OFF_BAR = OFF_BB + (size_t)NB * BSLOT * sizeof(T);
-    static constexpr size_t BYTES = OFF_BAR + (size_t)(R + RB + NB) * 8 + 128;
+    static constexpr size_t BYTES = OFF_BAR + (size_t)(R + NB) * 8 + 128;
 };
 
 template <typename T, int TY, int R, int RB, int NB>
@@ -59,7 +61,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const T* sb = reinterpret_cast<const T*>(smem + L::OFF_B0);
     T* sB = reinterpret_cast<T*>(smem + L::OFF_BB);
     const uint32_t sx_u32 = ptx::smem_u32(sx), sb_u32 = ptx::smem_u32(sb);
-    const uint32_t bar_x = ptx::smem_u32(smem + L::OFF_BAR), bar_b = bar_x + 8u * R, bar_full = bar_b + 8u * RB;
+    const uint32_t bar_x = ptx::smem_u32(smem + L::OFF_BAR), bar_full = bar_x + 8u * R;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool tilew = warp < NTW;
@@ -70,12 +72,11 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int kend = min(k1, nz - 1);
     const int first_p = max(k0 - 1, 0);
     const int pfirst = max(first_p - 1, 0), plast = min(kend + 1, nz - 1);
-    const int bfirst = first_p, blast = kend;
     const T twoh[3] = { a.twoh[0], a.twoh[1], a.twoh[2] };
 
     const bool pwarp = warp == NW - 1, producer = pwarp && lane == 0;
     if (producer) {
-        for (int s = 0; s < R + RB; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
+        for (int s = 0; s < R; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
         for (int s = 0; s < NB; ++s) ptx::mbar_init(bar_full + 8u * s, NW);      // one arrival per warp
         ptx::fence_mbar_init();
     }
@@ -85,22 +86,17 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     tmem::fence_after_sync();
     const uint32_t tm0 = tm_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * WCOLS);
 
-    auto load_x = [&](int p) {
-        const uint32_t s = (uint32_t)((p - pfirst) % R);
-        ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES);
-        ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, p, 0, bar_x + 8u * s);
+    // one ring position and one mbarrier per plane for the xi box and the b box (they are born and die together)
+    int next_x = pfirst;
+    auto refill = [&](int upto) {
+        for (const int last = min(upto, plast); next_x <= last; ++next_x) {
+            const uint32_t s = (uint32_t)((next_x - pfirst) % R);
+            ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES + L::BBOX_BYTES);
+            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, next_x, 0, bar_x + 8u * s);
+            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, next_x, 0, bar_x + 8u * s);
+        }
     };
-    auto load_b = [&](int p) {
-        const uint32_t s = (uint32_t)((p - bfirst) % RB);
-        ptx::mbar_expect_tx(bar_b + 8u * s, L::BBOX_BYTES);
-        ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, p, 0, bar_b + 8u * s);
-    };
-    int next_x = pfirst, next_b = bfirst;
-    auto refill = [&](int upto_x, int upto_b) {
-        for (const int last = min(upto_x, plast); next_x <= last; ++next_x) load_x(next_x);
-        for (const int last = min(upto_b, blast); next_b <= last; ++next_b) load_b(next_b);
-    };
-    if (producer) refill(pfirst + R - 1, bfirst + RB - 1);
+    if (producer) refill(pfirst + R - 1);
 
     // the node of this thread: tile warps own the row `warp` of the tile; R-warps a node of the halo-1 ring (row below,
     // row above, both columns) or none (the producer's warp)
@@ -138,19 +134,18 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     uint32_t rp = 0u;                             // TMEM record buffer of the plane p
     int s0 = (first_p - pfirst) % R, s1 = (s0 + 1) % R, s2 = (s0 + 2) % R, sm1 = (s0 + R - 1) % R, sm2 = (s0 + R - 2) % R;
     uint32_t par1 = (uint32_t)(((first_p + 1 - pfirst) / R) & 1);
-    int sb0 = 0;
-    uint32_t parb = 0u;
     T x1[3] = { T(0), T(0), T(0) };
+  auto run = [&](auto tile_c) {
+    constexpr bool TILE = decltype(tile_c)::value;
 #pragma unroll 1
     for (int p = first_p; p <= kend; ++p) {
         const T* f1 = sx + s0 * L::SLOTX;                     // xi plane p
         const T* f2 = sx + s1 * L::SLOTX;                     // xi plane p+1
         if (p + 1 <= plast) ptx::mbar_wait(bar_x + 8u * (uint32_t)s1, par1);
-        ptx::mbar_wait(bar_b + 8u * (uint32_t)sb0, parb);
-        const T* bs = sb + sb0 * L::SLOTB;
+        const T* bs = sb + s0 * L::SLOTB;
         // ---------------- A(p): push-forward of the plane p at the own node ----------------
         T Bp[3] = { T(0), T(0), T(0) };
-        if (tilew || (has_node && p >= k0 && p < kend)) {
+        if (TILE || (has_node && p >= k0 && p < kend)) {
             T dF[3][3];
             const T* fr = f1 + ox;
 #pragma unroll
@@ -178,7 +173,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             d[0] = Bp[0];
             d[BCS] = Bp[1];
             d[2 * BCS] = Bp[2];
-            if (tilew) {
+            if constexpr (TILE) {
                 const T sn = (p > 0 && p < nz - 1 && in_xy) ? a.dtg * inv : T(0);
                 uint32_t w0[CW], w1[CW];
 #pragma unroll
@@ -196,16 +191,16 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 if constexpr (CW == 16) { tmem::st16(ra, w0); tmem::st16(ra + CW, w1); }
                 else { tmem::st8(ra, w0); tmem::st8(ra + CW, w1); }
             }
-        } else if (has_node) {
+        } else if (!TILE && has_node) {
             const T* fr = f1 + ox;
 #pragma unroll
             for (int c = 0; c < 3; ++c) x1[c] = fr[c * CSX];
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar_full + 8u * (uint32_t)buf);      // this warp's part of B(p) is in shared memory
-        if (pwarp) {
+        if (!TILE && pwarp) {
             ptx::named_sync(BAR_A + buf, NW * 32);            // every warp is done with the xi / b planes p
-            if (producer) refill(p + R, p + RB);
+            if (producer) refill(p + R);
         } else {
             ptx::named_arrive(BAR_A + buf, NW * 32);
         }
@@ -213,7 +208,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         if (p > first_p) {
             ptx::mbar_wait(bar_full + 8u * (uint32_t)pb, ppar);   // every warp has published B(p-1) (about an iteration ago)
             const int t = p - 1;
-            if (tilew && t >= k0) {
+            if (TILE && t >= k0) {
                 uint32_t w0[CW], w1[CW];
                 const uint32_t ra = tm0 + (rp ^ 1u) * REC;
                 if constexpr (CW == 16) { tmem::ld16(ra, w0); tmem::ld16(ra + CW, w1); }
@@ -260,15 +255,17 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         }
 #pragma unroll
         for (int c = 0; c < 3; ++c) { Bm[c] = Bc[c]; Bc[c] = Bp[c]; xc[c] = x1[c]; }
-        tmem::wait_st();                                      // record(p) is complete before the next iteration reads it
+        if constexpr (TILE) tmem::wait_st();                  // record(p) is complete before the next iteration reads it
         pb = buf; ppar = cpar;
         if (++buf == NB) { buf = 0; cpar ^= 1u; }
         rp ^= 1u;
         sm2 = sm1; sm1 = s0; s0 = s1; s1 = s2;
         if (s1 == 0) par1 ^= 1u;
         if (++s2 == R) s2 = 0;
-        if (++sb0 == RB) { sb0 = 0; parb ^= 1u; }
     }
+  };
+  if (tilew) run(std::true_type{});
+  else run(std::false_type{});
     if (k1 == nz && st) {   // the top plane (line-tied) is carried through
         T* pl = out + (long long)(nz - 1) * a.plane + (long long)gj * a.pitch + gi;
         pl[0] = x1[0];
@@ -283,7 +280,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 
 // ----------------------------------------------------------------------------------------------- host side
 
-constexpr int kSTY = 16, kSR = 5, kSRB = 3, kSNB = 4;
+constexpr int kSTY = 16, kSR = 4, kSRB = 4, kSNB = 4;
 
 inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* xi0, void* xi1, void* b, int sm_count,
                            std::string* why)
