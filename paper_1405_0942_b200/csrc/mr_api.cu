@@ -224,7 +224,7 @@ mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
 {
     const bool mim = op == MR_OP_MIMETIC;
     const int fv = c->force_variant;
-    const bool use_sym = mim && fv == 7 && c->plan7.usable;
+    const bool use_sym = mim && (fv == 0 || fv == 7) && c->plan7.usable;
     const bool use_duo = mim && !use_sym && (fv == 0 || fv == 6) && c->plan5.usable;
     const bool use_park = mim && !use_duo && fv == 5 && c->plan4.usable;           // experimental variants: only when forced
     const bool use_lean = mim && !use_park && fv == 4 && c->plan3.usable;
@@ -277,7 +277,7 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     const T* b = static_cast<const T*>(c->b());
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     const int threads = c->grid.nx >= 256 ? 256 : (c->grid.nx >= 128 ? 128 : (c->grid.nx >= 64 ? 64 : 32));
-    const bool fused = op == MR_OP_MIMETIC && c->plan5.usable && (c->force_variant == 0 || c->force_variant == 6) &&
+    const bool fused = op == MR_OP_MIMETIC && c->plan5.usable && (c->force_variant == 0 || c->force_variant >= 6) &&
                        c->plan5.tiles_x * c->plan5.tiles_y * c->plan5.nchunks <= kMaxPartialBlocks;
     if (fused) {
         // the streaming pass of the step kernel with the update replaced by the reduction (mr_duo.cuh, DIAG)
