@@ -111,7 +111,7 @@ def test_fields_match_oracle(mr, name, op):
 
 @pytest.mark.parametrize("name", CASES)
 @pytest.mark.parametrize("op", ["mimetic", "direct"])
-@pytest.mark.parametrize("variant", ["auto", "generic", "stream", "pair", "lean", "park", "duo", "sym"])
+@pytest.mark.parametrize("variant", ["auto", "generic", "stream", "pair", "lean", "park", "duo", "sym", "sym2"])
 def test_one_step_matches_oracle(mr, name, op, variant):
     """S1-S5 fused: x after one step, also measured on the displacement moved in that step.  Every step-kernel
     variant of the library is held to the same bar ("auto" is the one the bench times)."""
