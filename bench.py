@@ -299,7 +299,7 @@ def run_ours(args):
 
     if rank == 0:
         line = {
-            "metric": METRIC if op == "mimetic" else METRIC.replace("mimetic", "direct"), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "metric": (METRIC if op == "mimetic" else METRIC.replace("mimetic", "direct")).replace("fp64", "fp64" if dtype == "f64" else "fp32"), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": dtype, "data": "synthetic",
             "config": {"workload": "%s %dx%dx%d %s %s, line-tied, forward Euler dt=%.3e" % ((cfg.name,) + g.n + ("fp64" if dtype == "f64" else "fp32", op, dt)),
