@@ -323,7 +323,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5"])
-    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "stream", "pair", "lean", "park", "duo", "sym", "sym2"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "generic"])
     ap.add_argument("--operator", default="mimetic", choices=["mimetic", "direct"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -126,11 +126,9 @@ const char* mr_last_error(const mr_ctx* ctx);
 int64_t mr_launch_count(const mr_ctx* ctx);
 const char* mr_step_variant(const mr_ctx* ctx);
 
-/* Choose the step kernel.  "auto" (default): mimetic operator -> the symmetric split-phase streaming kernel
- * ("sym"), direct operator -> the streaming kernel of mr_direct.cuh.  "generic": always the global-memory kernel
- * (the A/B reference, both operators).  "stream", "pair", "lean", "park", "duo", "sym", "sym2": force one of the
- * streaming kernels of the mimetic operator (DESIGN.md section 6 tells them apart); mr_step then fails with
- * MR_ERR_INVALID_ARG for the direct operator.  All variants agree to rounding ("duo", "sym", "sym2" bit for bit). */
+/* Choose the step kernel.  "auto" (default): the streaming TMA kernels (mimetic: csrc/mr_sym.cuh, direct:
+ * csrc/mr_direct.cuh).  "generic": the global-memory kernels of csrc/mr_generic.cuh for both operators (one thread per
+ * node, every stencil value straight from global memory): the A/B reference of the tests.  Both agree to rounding. */
 mr_status mr_set_variant(mr_ctx* ctx, const char* name);
 
 #ifdef __cplusplus

@@ -9,14 +9,10 @@
 
 #include "mr_common.cuh"
 #include "mr_generic.cuh"
-#include "mr_stream.cuh"
-#include "mr_pair.cuh"
-#include "mr_lean.cuh"
-#include "mr_park.cuh"
+#include "mr_stream_common.cuh"
 #include "mr_duo.cuh"
 #include "mr_direct.cuh"
 #include "mr_sym.cuh"
-#include "mr_sym2.cuh"
 
 using namespace mr;
 
@@ -78,16 +74,11 @@ struct mr_ctx {
     int64_t steps;
     int64_t launches;
     int sm_count;
-    int force_variant;  // 0 auto, 1 generic, 2 stream, 3 pair, 4 lean, 5 park, 6 duo, 7 sym, 8 sym2
+    int force_variant;  // 0 auto (streaming kernels), 1 generic (global-memory kernels, the A/B reference)
     const char* variant;
-    StreamPlan plan;    // TMA descriptors etc. for the first streaming kernel (mr_stream.cuh)
-    StreamPlan plan2;   // ... for the register-paired streaming kernel (mr_pair.cuh)
-    StreamPlan plan3;   // ... for the lean-state streaming kernel (mr_lean.cuh)
-    StreamPlan plan4;   // ... for the TMEM-parked streaming kernel (mr_park.cuh)
-    StreamPlan plan5;   // ... and for the warp-specialised streaming kernel (mr_duo.cuh)
+    StreamPlan plan5;   // TMA descriptors etc. of the warp-specialised streaming pass (mr_duo.cuh; S6 of the mimetic operator)
     StreamPlan plan6;   // the streaming kernel of the direct-derivative operator (mr_direct.cuh)
-    StreamPlan plan7;   // the symmetric split-phase streaming kernel (mr_sym.cuh)
-    StreamPlan plan8;   // ... with two rows per tile warp (mr_sym2.cuh, experiment)
+    StreamPlan plan7;   // the symmetric split-phase streaming kernel of the mimetic operator (mr_sym.cuh)
     std::string err;
 
     void* xi(int w) const { return ws + L.off_xi[w]; }
@@ -225,31 +216,15 @@ template <typename T>
 mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
 {
     const bool mim = op == MR_OP_MIMETIC;
-    const int fv = c->force_variant;
-    const bool use_sym2 = mim && fv == 8 && c->plan8.usable;
-    const bool use_sym = mim && !use_sym2 && (fv == 0 || fv == 7) && c->plan7.usable;
-    const bool use_duo = mim && !use_sym2 && !use_sym && (fv == 0 || fv == 6) && c->plan5.usable;
-    const bool use_park = mim && !use_duo && fv == 5 && c->plan4.usable;           // experimental variants: only when forced
-    const bool use_lean = mim && !use_park && fv == 4 && c->plan3.usable;
-    const bool use_pair = mim && !use_duo && !use_park && !use_lean && (fv == 0 || fv == 3) && c->plan2.usable;
-    const bool use_stream = mim && !use_duo && !use_park && !use_lean && !use_pair && (fv == 0 || fv == 2) && c->plan.usable;
-    if ((fv == 2 && !use_stream) || (fv == 3 && !use_pair) || (fv == 4 && !use_lean) || (fv == 5 && !use_park) || (fv == 6 && !use_duo) || (fv == 7 && !use_sym) || (fv == 8 && !use_sym2))
-        return fail(c, MR_ERR_INVALID_ARG, "mr_step: a streaming kernel was forced but does not take this grid/operator");
-    const bool use_dstream = !mim && fv == 0 && c->plan6.usable;
-    c->variant = use_dstream ? c->plan6.name : use_sym2 ? c->plan8.name : use_sym ? c->plan7.name : use_duo ? c->plan5.name : use_park ? c->plan4.name : use_lean ? c->plan3.name : use_pair ? c->plan2.name : use_stream ? c->plan.name
-                 : (mim ? "generic_mimetic" : "generic_direct");
+    const bool use_sym = mim && c->force_variant == 0 && c->plan7.usable;
+    const bool use_dstream = !mim && c->force_variant == 0 && c->plan6.usable;
+    c->variant = use_dstream ? c->plan6.name : use_sym ? c->plan7.name : (mim ? "generic_mimetic" : "generic_direct");
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     for (int64_t s = 0; s < n; ++s) {
-        if (use_dstream || use_sym2 || use_sym || use_duo || use_park || use_lean || use_pair || use_stream) {
+        if (use_dstream || use_sym) {
             const T dtg = (T)(dt * c->gamma);
             cudaError_t e = use_dstream ? launch_direct_step<T>(c->plan6, c->cur, dtg, c->flag(), c->stream)
-                            : use_sym2 ? launch_sym2_step<T>(c->plan8, c->cur, dtg, c->flag(), c->stream)
-                            : use_sym ? launch_sym_step<T>(c->plan7, c->cur, dtg, c->flag(), c->stream)
-                            : use_duo ? launch_duo_step<T>(c->plan5, c->cur, dtg, c->flag(), c->stream)
-                            : use_park ? launch_park_step<T>(c->plan4, c->cur, dtg, c->flag(), c->stream)
-                            : use_lean ? launch_lean_step<T>(c->plan3, c->cur, dtg, c->flag(), c->stream)
-                            : use_pair ? launch_pair_step<T>(c->plan2, c->cur, dtg, c->flag(), c->stream)
-                                       : launch_stream_step<T>(c->plan, c->cur, dtg, c->flag(), c->stream);
+                                        : launch_sym_step<T>(c->plan7, c->cur, dtg, c->flag(), c->stream);
             if (e != cudaSuccess) return cuda_fail(c, "streaming step launch", e);
             c->launches++;
         } else {
@@ -281,7 +256,7 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     const T* b = static_cast<const T*>(c->b());
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     const int threads = c->grid.nx >= 256 ? 256 : (c->grid.nx >= 128 ? 128 : (c->grid.nx >= 64 ? 64 : 32));
-    const bool fused = op == MR_OP_MIMETIC && c->plan5.usable && (c->force_variant == 0 || c->force_variant >= 6) &&
+    const bool fused = op == MR_OP_MIMETIC && c->plan5.usable && c->force_variant == 0 &&
                        c->plan5.tiles_x * c->plan5.tiles_y * c->plan5.nchunks <= kMaxPartialBlocks;
     if (fused) {
         // the streaming pass of the step kernel with the update replaced by the reduction (mr_duo.cuh, DIAG)
@@ -378,22 +353,6 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     sg.pitch = L.pitch; sg.plane = L.plane; sg.comp = L.comp;
     for (int a = 0; a < 3; ++a) sg.twoh[a] = 2.0 * c->h[a];
     std::string why;
-    if (!build_stream_plan(&c->plan, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan.usable = false;
-        c->plan.why = why;
-    }
-    if (!build_pair_plan(&c->plan2, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan2.usable = false;
-        c->plan2.why = why;
-    }
-    if (!build_lean_plan(&c->plan3, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan3.usable = false;
-        c->plan3.why = why;
-    }
-    if (!build_park_plan(&c->plan4, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan4.usable = false;
-        c->plan4.why = why;
-    }
     if (!build_duo_plan(&c->plan5, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
         c->plan5.usable = false;
         c->plan5.why = why;
@@ -405,10 +364,6 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     if (!build_sym_plan(&c->plan7, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
         c->plan7.usable = false;
         c->plan7.why = why;
-    }
-    if (!build_sym2_plan(&c->plan8, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan8.usable = false;
-        c->plan8.why = why;
     }
     *out = c;
     return MR_OK;
@@ -510,13 +465,6 @@ extern "C" mr_status mr_set_variant(mr_ctx* ctx, const char* name)
     if (!ctx || !name) return MR_ERR_INVALID_ARG;
     if (!std::strcmp(name, "auto")) ctx->force_variant = 0;
     else if (!std::strcmp(name, "generic")) ctx->force_variant = 1;
-    else if (!std::strcmp(name, "stream")) ctx->force_variant = 2;
-    else if (!std::strcmp(name, "pair")) ctx->force_variant = 3;
-    else if (!std::strcmp(name, "lean")) ctx->force_variant = 4;
-    else if (!std::strcmp(name, "park")) ctx->force_variant = 5;
-    else if (!std::strcmp(name, "duo")) ctx->force_variant = 6;
-    else if (!std::strcmp(name, "sym")) ctx->force_variant = 7;
-    else if (!std::strcmp(name, "sym2")) ctx->force_variant = 8;
-    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto, generic, stream, pair, lean, park or duo");
+    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto or generic");
     return MR_OK;
 }

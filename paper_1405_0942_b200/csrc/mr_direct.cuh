@@ -10,7 +10,8 @@
 // synchronisation is the recycling of the ring slots: every warp arrives on a named barrier when it is done with
 // the plane k-1, only the producer's warp waits on it.
 #pragma once
-#include "mr_duo.cuh"
+#include "mr_generic.cuh"
+#include "mr_stream_common.cuh"
 
 namespace mr {
 

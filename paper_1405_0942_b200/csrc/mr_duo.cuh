@@ -27,7 +27,7 @@
 #include <type_traits>
 
 #include "mr_generic.cuh"
-#include "mr_pair.cuh"
+#include "mr_stream_common.cuh"
 #include "mr_tmem.cuh"
 
 namespace mr {
@@ -54,35 +54,6 @@ struct DuoLayout {
     static constexpr size_t OFF_BAR = OFF_BB + (size_t)NB * BSLOT * sizeof(T);
     static constexpr size_t BYTES = OFF_BAR + (size_t)(R + RB) * 8 + 128;   // +128: base alignment slack
 };
-
-namespace ptx {
-__device__ __forceinline__ void named_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory"); }
-__device__ __forceinline__ void named_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
-}  // namespace ptx
-
-// The A-warp's share of stage A at one node: dF comes in without the 2h diagonal and leaves with it; n_0 = dF_1 x dF_2
-// (area vector of the jk index surface, Eqs. 2.5/2.6), D = det dF = dF_0 . n_0, inv = 1/D, B = dF b / D (Eq. 2.1).
-// n_1 and n_2 are formed by the F-warp from the columns of dF.
-template <typename T, int CSB>
-__device__ __forceinline__ void duo_push(T (&dF)[3][3], const T* __restrict__ bs, const T (&twoh)[3], T (&n0)[3], T (&B)[3], T& inv,
-                                         bool& ok, bool in_dom)
-{
-#pragma unroll
-    for (int c = 0; c < 3; ++c) dF[c][c] += twoh[c];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
-        n0[c] = dF[c1][1] * dF[c2][2] - dF[c2][1] * dF[c1][2];
-    }
-    const T D = dF[0][0] * n0[0] + dF[1][0] * n0[1] + dF[2][0] * n0[2];
-    ok = ok && (positive_finite(D) || !in_dom);
-    inv = fast_rcp(D);
-    // dF b first, the division last: the nine products do not wait for the reciprocal's Newton chain
-    const T b0 = bs[0], b1 = bs[CSB], b2 = bs[2 * CSB];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) B[c] = (dF[c][0] * b0 + dF[c][1] * b1 + dF[c][2] * b2) * inv;
-}
 
 template <typename T, int TY, int R, int RB, int NB, bool DIAG>
 #ifndef MR_DUO_MAXREG

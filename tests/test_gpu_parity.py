@@ -111,12 +111,10 @@ def test_fields_match_oracle(mr, name, op):
 
 @pytest.mark.parametrize("name", CASES)
 @pytest.mark.parametrize("op", ["mimetic", "direct"])
-@pytest.mark.parametrize("variant", ["auto", "generic", "stream", "pair", "lean", "park", "duo", "sym", "sym2"])
+@pytest.mark.parametrize("variant", ["auto", "generic"])
 def test_one_step_matches_oracle(mr, name, op, variant):
     """S1-S5 fused: x after one step, also measured on the displacement moved in that step.  Every step-kernel
     variant of the library is held to the same bar ("auto" is the one the bench times)."""
-    if op == "direct" and variant not in ("auto", "generic"):
-        pytest.skip("the streaming kernels implement the mimetic operator only")
     g, x0, B0, dt = case(name)
     sim = make_sim(mr, g, x0, B0, variant=variant)
     sim.step(1, dt, op)
@@ -133,7 +131,7 @@ def test_one_step_matches_oracle(mr, name, op, variant):
 
 
 @pytest.mark.parametrize("name,steps", [("C1", 100), ("C2_small", 100), ("C3_small", 100), ("ragged", 100)])
-@pytest.mark.parametrize("variant", ["auto", "generic", "stream", "pair", "duo", "sym"])
+@pytest.mark.parametrize("variant", ["auto", "generic"])
 def test_100_steps_match_oracle(mr, name, steps, variant):
     g, x0, B0, dt = case(name)
     sim = make_sim(mr, g, x0, B0, variant=variant)
@@ -209,7 +207,7 @@ def test_abc_on_undistorted_grid_does_not_move(mr):
     assert sim.diagnostics()["max_jxb"] < 1e-11
 
 
-@pytest.mark.parametrize("variant", ["auto", "generic", "stream", "pair", "duo", "sym"])
+@pytest.mark.parametrize("variant", ["auto", "generic"])
 def test_fp32_variant_within_1e5_of_fp64(mr, variant):
     """fp32 storage+arithmetic (displacement storage, Q15) against the fp64 GPU run and the fp64 oracle."""
     cfg = I.scaled(I.CONFIGS["C5"], (64, 64, 64))
