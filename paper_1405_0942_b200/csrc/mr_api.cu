@@ -10,7 +10,6 @@
 #include "mr_common.cuh"
 #include "mr_generic.cuh"
 #include "mr_stream_common.cuh"
-#include "mr_duo.cuh"
 #include "mr_direct.cuh"
 #include "mr_sym.cuh"
 
@@ -76,7 +75,6 @@ struct mr_ctx {
     int sm_count;
     int force_variant;  // 0 auto (streaming kernels), 1 generic (global-memory kernels, the A/B reference)
     const char* variant;
-    StreamPlan plan5;   // TMA descriptors etc. of the warp-specialised streaming pass (mr_duo.cuh; S6 of the mimetic operator)
     StreamPlan plan6;   // the streaming kernel of the direct-derivative operator (mr_direct.cuh)
     StreamPlan plan7;   // the symmetric split-phase streaming kernel of the mimetic operator (mr_sym.cuh)
     std::string err;
@@ -256,11 +254,11 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     const T* b = static_cast<const T*>(c->b());
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     const int threads = c->grid.nx >= 256 ? 256 : (c->grid.nx >= 128 ? 128 : (c->grid.nx >= 64 ? 64 : 32));
-    const bool fused = op == MR_OP_MIMETIC && c->plan5.usable && c->force_variant == 0 &&
-                       c->plan5.tiles_x * c->plan5.tiles_y * c->plan5.nchunks <= kMaxPartialBlocks;
+    const bool fused = op == MR_OP_MIMETIC && c->plan7.usable && c->force_variant == 0 &&
+                       c->plan7.tiles_x * c->plan7.tiles_y * c->plan7.nchunks <= kMaxPartialBlocks;
     if (fused) {
-        // the streaming pass of the step kernel with the update replaced by the reduction (mr_duo.cuh, DIAG)
-        cudaError_t e = launch_duo_diag<T>(c->plan5, c->cur, c->partials(), &blocks, c->flag(), c->stream);
+        // the streaming pass of the step kernel with the update replaced by the reduction (mr_sym.cuh, DIAG)
+        cudaError_t e = launch_sym_diag<T>(c->plan7, c->cur, c->partials(), &blocks, c->flag(), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, "streaming diagnostics launch", e);
     } else if (op == MR_OP_MIMETIC)
         k_diag<T, 0><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());
@@ -353,10 +351,6 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     sg.pitch = L.pitch; sg.plane = L.plane; sg.comp = L.comp;
     for (int a = 0; a < 3; ++a) sg.twoh[a] = 2.0 * c->h[a];
     std::string why;
-    if (!build_duo_plan(&c->plan5, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan5.usable = false;
-        c->plan5.why = why;
-    }
     if (!build_direct_plan(&c->plan6, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
         c->plan6.usable = false;
         c->plan6.why = why;

@@ -1,27 +1,35 @@
-// mr_sym.cuh -- the symmetric split-phase streaming step kernel for the mimetic operator (S1-S5 in one pass).
+// mr_sym.cuh -- the streaming step kernel of the mimetic operator (S1-S5 in one pass) and, as its DIAG
+// instantiation, the grid-wide reduction S6 by the same pass.
 //
-// Same ingredients as mr_duo.cuh (TMA rings of xi and b, B shared through shared-memory planes, the node's record
-// parked in Tensor Memory, dedicated warps for the halo-1 ring), but without roles: each of the 16 tile warps owns one
-// row of the 32 x 16 tile (one node per thread) and in iteration p does
-//     A(p):    dF, n_0, D, 1/D, B(p) = dF b / D (Eq. 2.1) -> shared B plane p % NB;  record(p) -> TMEM (own columns);
-//              mbarrier.arrive FULL[p % NB]
-//     F(p-1):  mbarrier wait FULL[(p-1) % NB] -- a phase that completed about one iteration ago, so the wait is a
-//              poll, not a stall --, D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x (B(p) - B(p-2)) (closed form of
-//              Eqs. 2.3-2.7), u = gamma J x B (Eq. 1.5), xi+ = xi + dt u -> HBM.
-// The two halves of an iteration belong to different planes and are independent: every warp carries the same load
-// (no A/F imbalance), and nobody waits for the slowest warp of the current plane.  A buffer p % NB is overwritten
-// NB planes later; a warp that starts A(p) has seen FULL[p-2] complete, i.e. every warp has finished F(p-4): NB = 4.
+// Work item = (32 x 16 xy tile, chunk of z-planes); a CTA marches along k.  Per plane the TMA unit streams the box of
+// xi (halo 2 in j, 16 bytes in i) and of b (halo 1) into one of four shared-memory ring positions.  Each of the 16
+// tile warps owns one row of the tile (one node per thread); four more warps own the halo-1 ring of the tile (row
+// below, row above, both columns; only B is formed there) and the TMA producer.  In iteration p a tile warp does
+//     A(p):    dF, n_0 = dF_1 x dF_2, D = dF_0 . n_0, 1/D, B(p) = dF b / D (Eq. 2.1) -> shared B plane p % 4;
+//              record(p) = (dF, n_0) -> Tensor Memory (own columns);  mbarrier.arrive FULL[p % 4]
+//     F(p-1):  wait FULL[(p-1) % 4] -- a phase that completed about one iteration ago --,
+//              D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x (B(p) - B(p-2))   (closed form of Eqs. 2.3-2.7),
+//              u = gamma J x B (Eq. 1.5), xi+ = xi + dt u -> HBM          (DIAG: the reduction of S6 instead).
+// The two halves belong to different planes and are independent: every warp carries the same load and nobody waits
+// for the slowest warp of the current plane.  A warp that starts A(p) has seen FULL[p-2] complete, i.e. every warp has
+// finished F(p-4): four B planes suffice.
+//
+// The k loop is unrolled by four with the phase q = (p - first_p) % 4 a compile-time constant: every ring position,
+// B plane, barrier, TMEM record and the rotating register sets (own B of the last planes: period 4, own xi: period 2)
+// are named at compile time, so the loop carries no register moves and no address arithmetic (ncu of the rolled loop:
+// 82 of its 356 instructions per node were moves, profiles/r1f_full.md).
 #pragma once
 #include <type_traits>
 
-#include "mr_duo.cuh"
+#include "mr_generic.cuh"
+#include "mr_stream_common.cuh"
+#include "mr_tmem.cuh"
 
 namespace mr {
 
-template <typename T, int TY, int R, int RB, int NB>
+template <typename T>
 struct SymLayout {
-    static_assert(TY == 16 && R >= 4 && RB == R && NB >= 4, "tile / ring sizes (xi and b share the ring positions)");
-    static constexpr int TX = 32;
+    static constexpr int TX = 32, TY = 16, R = 4, NB = 4;
     static constexpr int HXL = 16 / (int)sizeof(T), HXR = 2 * HXL;
     static constexpr int BW = TX + HXL + HXR;
     static constexpr int XH = TY + 4, BH = TY + 2;
@@ -33,27 +41,31 @@ struct SymLayout {
     static constexpr int BBW = TX + 2, BBH = TY + 2;
     static constexpr int BCS = BBW * BBH;
     static constexpr int BSLOT = round128(3 * BCS * (int)sizeof(T)) / (int)sizeof(T);
-    static constexpr int NTW = TY, NWARPS = TY + 4, NTHREADS = NWARPS * 32;     // tile warps + 4 R-warps
+    static constexpr int NTW = TY, NWARPS = TY + 4, NTHREADS = NWARPS * 32;     // tile warps + 4 ring warps
     static constexpr size_t OFF_X = 0;
     static constexpr size_t OFF_B0 = OFF_X + (size_t)R * SLOTX * sizeof(T);
-    static constexpr size_t OFF_BB = OFF_B0 + (size_t)RB * SLOTB * sizeof(T);
+    static constexpr size_t OFF_BB = OFF_B0 + (size_t)R * SLOTB * sizeof(T);
     static constexpr size_t OFF_BAR = OFF_BB + (size_t)NB * BSLOT * sizeof(T);
     static constexpr size_t BYTES = OFF_BAR + (size_t)(R + NB) * 8 + 128;
+    // TMEM record of a node: chunk 0 = columns 0, 1 of dF, n_0[0], n_0[1] (8 values), chunk 1 = column 2 of dF, n_0[2]
+    static constexpr int WN = (int)sizeof(T) / 4;                   // 32-bit words per value
+    static constexpr int C0W = 8 * WN, C1W = 4 * WN, REC = 16 * WN; // record stride (12 values, padded to 16)
+    static constexpr int TMEM_COLS = (NTW / 4) * 2 * REC;           // warps of a lane quarter x two records (plane parity)
 };
 
-template <typename T, int TY, int R, int RB, int NB>
+template <int Q> using Phase = std::integral_constant<int, Q>;
+
+template <typename T, bool DIAG>
 __global__ void __maxnreg__(96)
 k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, T* __restrict__ out,
            const StreamArgs<T> a)
 {
-    using L = SymLayout<T, TY, R, RB, NB>;
+    using L = SymLayout<T>;
     using W32 = tmem::Words<T>;
-    constexpr int TX = L::TX, NTW = L::NTW, BW = L::BW, CSX = L::CSX, CSB = L::CSB, BBW = L::BBW, BCS = L::BCS;
-    constexpr int NW = L::NWARPS;
-    constexpr int CW = 8 * W32::N, REC = 2 * CW;                   // record: 16 values in two chunks
-    constexpr int WCOLS = 2 * REC;                                  // two record buffers (plane parity) per tile warp
-    static_assert((NTW / 4) * WCOLS <= 512, "TMEM columns");
-    constexpr int BAR_A = 1;                                        // named barriers BAR_A .. BAR_A + NB - 1
+    constexpr int TX = L::TX, TY = L::TY, NTW = L::NTW, BW = L::BW, CSX = L::CSX, CSB = L::CSB, BBW = L::BBW, BCS = L::BCS;
+    constexpr int NW = L::NWARPS, WN = L::WN, C0W = L::C0W, C1W = L::C1W, REC = L::REC;
+    static_assert(L::TMEM_COLS == 256 || L::TMEM_COLS == 128, "TMEM columns: a power of two");
+    constexpr int BAR_A = 1;                                        // named barriers BAR_A .. BAR_A + 3
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t tm_base_s;
     unsigned char* smem = smem_raw + ((128u - (ptx::smem_u32(smem_raw) & 127u)) & 127u);
@@ -61,7 +73,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const T* sb = reinterpret_cast<const T*>(smem + L::OFF_B0);
     T* sB = reinterpret_cast<T*>(smem + L::OFF_BB);
     const uint32_t sx_u32 = ptx::smem_u32(sx), sb_u32 = ptx::smem_u32(sb);
-    const uint32_t bar_x = ptx::smem_u32(smem + L::OFF_BAR), bar_full = bar_x + 8u * R;
+    const uint32_t bar_x = ptx::smem_u32(smem + L::OFF_BAR), bar_full = bar_x + 8u * L::R;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool tilew = warp < NTW;
@@ -69,36 +81,45 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY;
     const int nz = a.nz;
     const int k0 = chunk * a.chunk_len, k1 = min(k0 + a.chunk_len, nz);
-    const int kend = min(k1, nz - 1);
-    const int first_p = max(k0 - 1, 0);
-    const int pfirst = max(first_p - 1, 0), plast = min(kend + 1, nz - 1);
+    const int kend = min(k1, nz - 1);               // planes k0 .. kend-1 are finished here (and nz-1 carried through)
+    const int first_p = max(k0 - 1, 0);             // B is formed on the planes first_p .. kend
+    const int pfirst = max(first_p - 1, 0), plast = min(kend + 1, nz - 1);       // xi / b planes this item touches
     const T twoh[3] = { a.twoh[0], a.twoh[1], a.twoh[2] };
 
     const bool pwarp = warp == NW - 1, producer = pwarp && lane == 0;
     if (producer) {
-        for (int s = 0; s < R; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
-        for (int s = 0; s < NB; ++s) ptx::mbar_init(bar_full + 8u * s, NW);      // one arrival per warp
+        for (int s = 0; s < L::R; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
+        for (int s = 0; s < L::NB; ++s) ptx::mbar_init(bar_full + 8u * s, NW);   // one arrival per warp
         ptx::fence_mbar_init();
     }
-    if (warp == 0) tmem::alloc<512>(&tm_base_s);
+    if (warp == 0) tmem::alloc<L::TMEM_COLS>(&tm_base_s);
     tmem::fence_before_sync();
     __syncthreads();
     tmem::fence_after_sync();
-    const uint32_t tm0 = tm_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * WCOLS);
+    const uint32_t tm0 = tm_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 2 * REC);
 
-    // one ring position and one mbarrier per plane for the xi box and the b box (they are born and die together)
+    // Ring position of the plane p: (p - first_p + 1) % 4, one mbarrier per position for the xi box and the b box (they
+    // are born and die together).  The plane nz does not exist: it is "delivered" empty, so that the consumers wait for
+    // the plane p+1 unconditionally.
     int next_x = pfirst;
     auto refill = [&](int upto) {
-        for (const int last = min(upto, plast); next_x <= last; ++next_x) {
-            const uint32_t s = (uint32_t)((next_x - pfirst) % R);
-            ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES + L::BBOX_BYTES);
-            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, next_x, 0, bar_x + 8u * s);
-            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, next_x, 0, bar_x + 8u * s);
+        for (; next_x <= upto; ++next_x) {
+            const uint32_t s = (uint32_t)(next_x - first_p + 1) & 3u;
+            if (next_x <= plast) {
+                ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES + L::BBOX_BYTES);
+                ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, next_x, 0, bar_x + 8u * s);
+                ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, next_x, 0, bar_x + 8u * s);
+            } else if (next_x == nz) {
+                ptx::mbar_arrive(bar_x + 8u * s);
+            }
         }
     };
-    if (producer) refill(pfirst + R - 1);
+    if (producer) {
+        if (first_p == 0) ptx::mbar_arrive(bar_x);          // position 0 would hold the plane -1: its first phase is empty
+        refill(pfirst + 3);
+    }
 
-    // the node of this thread: tile warps own the row `warp` of the tile; R-warps a node of the halo-1 ring (row below,
+    // the node of this thread: tile warps own the row `warp` of the tile; ring warps a node of the halo-1 ring (row below,
     // row above, both columns) or none (the producer's warp)
     int ti, tj;
     bool has_node = true;
@@ -108,112 +129,149 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     else if (warp == NTW + 2) { ti = (lane >> 3) & 1 ? TX : -1; tj = (lane & 7) + 8 * (lane >> 4); }
     else { ti = 0; tj = 0; has_node = false; }
     const int gi = i0 + ti, gj = j0 + tj;
-    const int ox = (tj + 2) * BW + (ti + L::HXL), ob = (tj + 1) * BW + (ti + L::HXL), oB = (tj + 1) * BBW + (ti + 1);
+    const T* px = sx + (tj + 2) * BW + (ti + L::HXL);       // this node in component 0 of the ring position 0 (xi, b, B)
+    const T* pb = sb + (tj + 1) * BW + (ti + L::HXL);
+    T* pB = sB + (tj + 1) * BBW + (ti + 1);
     const bool dom = has_node && gi >= 0 && gi < a.nx && gj >= 0 && gj < a.ny;
     const unsigned edge = !dom ? 0u : (gi == 0 ? 1u : 0u) | (gi == a.nx - 1 ? 2u : 0u) | (gj == 0 ? 4u : 0u) | (gj == a.ny - 1 ? 8u : 0u);
     const bool in_xy = gi > 0 && gi < a.nx - 1 && gj > 0 && gj < a.ny - 1;
     const bool st = tilew && dom;
 
-    auto wait_x = [&](int p) { const int q = p - pfirst; ptx::mbar_wait(bar_x + 8u * (uint32_t)(q % R), (uint32_t)((q / R) & 1)); };
-    for (int p = pfirst; p <= min(first_p + 1, plast); ++p) wait_x(p);
-    if (first_p == 0 && plast >= 2) wait_x(2);
+    // the planes first_p - 1 (own xi for the first k-difference), first_p and, for the one-sided difference on the bottom
+    // face, 2
+    if (first_p > 0) ptx::mbar_wait(bar_x, 0u);
+    ptx::mbar_wait(bar_x + 8u, 0u);
+    if (first_p == 0) ptx::mbar_wait(bar_x + 24u, 0u);
 
     bool ok = true;
-    T xc[3] = { T(0), T(0), T(0) };                              // own xi(p-1)
-    if (first_p > 0) {
-        const T* f = sx + ((first_p - 1 - pfirst) % R) * L::SLOTX + ox;
+    T xh[2][3], Bh[4][3], sh[2];                             // own xi(p), xi(p-1); own B(p) .. B(p-3); dt gamma / D of p, p-1
 #pragma unroll
-        for (int c = 0; c < 3; ++c) xc[c] = f[c * CSX];
+    for (int c = 0; c < 3; ++c) {
+        xh[0][c] = T(0);
+        xh[1][c] = first_p > 0 ? px[c * CSX] : T(0);        // phase 0 reads xi(first_p - 1) from xh[1]
+#pragma unroll
+        for (int q = 0; q < 4; ++q) Bh[q][c] = T(0);
     }
-    T Bm[3] = { T(0), T(0), T(0) }, Bc[3] = { T(0), T(0), T(0) };   // own B(p-2), B(p-1)
-    T xprev[3] = { T(0), T(0), T(0) };                              // unused placeholder to keep the layout of the loop simple
-    (void)xprev;
-    T* po = out + (long long)k0 * a.plane + (long long)gj * a.pitch + gi;     // plane t = p-1 of the first F
-    int buf = 0, pb = 0;                          // shared B plane of the plane p / p-1 (relative to first_p)
-    uint32_t cpar = 0u, ppar = 0u;                // phase parity of FULL[buf] for the plane p / p-1
-    uint32_t rp = 0u;                             // TMEM record buffer of the plane p
-    int s0 = (first_p - pfirst) % R, s1 = (s0 + 1) % R, s2 = (s0 + 2) % R, sm1 = (s0 + R - 1) % R, sm2 = (s0 + R - 2) % R;
-    uint32_t par1 = (uint32_t)(((first_p + 1 - pfirst) / R) & 1);
-    T x1[3] = { T(0), T(0), T(0) };
-  auto run = [&](auto tile_c) {
-    constexpr bool TILE = decltype(tile_c)::value;
-#pragma unroll 1
-    for (int p = first_p; p <= kend; ++p) {
-        const T* f1 = sx + s0 * L::SLOTX;                     // xi plane p
-        const T* f2 = sx + s1 * L::SLOTX;                     // xi plane p+1
-        if (p + 1 <= plast) ptx::mbar_wait(bar_x + 8u * (uint32_t)s1, par1);
-        const T* bs = sb + s0 * L::SLOTB;
+    sh[0] = sh[1] = T(0);
+    T* po = out + (long long)first_p * a.plane + (long long)gj * a.pitch + gi;     // plane t = p-1 of the first F
+    DiagPartial acc = { 0.0, 0.0, 0.0, INFINITY };          // DIAG: this thread's partial
+    const double zxy = ((gi == 0 || gi == a.nx - 1) ? 0.5 : 1.0) * ((gj == 0 || gj == a.ny - 1) ? 0.5 : 1.0);   // Eq. 3.13
+    auto diag_node = [&](int k, const T(&c0)[3], const T(&n0)[3], const T(&B)[3], const T(&uu)[3]) {
+        if (!st) return;
+        const double D = (double)c0[0] * n0[0] + (double)c0[1] * n0[1] + (double)c0[2] * n0[2];
+        const double b2 = (double)B[0] * B[0] + (double)B[1] * B[1] + (double)B[2] * B[2];
+        const bool kface = k == 0 || k == nz - 1;
+        DiagPartial v = { zxy * (kface ? 0.5 : 1.0) * b2 * D, 0.0, 0.0, D };
+        if (in_xy && !kface) {
+            const double fm = sqrt((double)uu[0] * uu[0] + (double)uu[1] * uu[1] + (double)uu[2] * uu[2]) / D;
+            v.fmax = fm;
+            v.xi = fm / b2;
+        }
+        diag_combine(acc, v);
+    };
+
+    int p = first_p;
+    uint32_t gpar = 0u;                                      // parity of the group of four planes
+    auto body = [&](auto phase, auto tile_c) {
+        constexpr int Q = decltype(phase)::value;
+        constexpr bool TILE = decltype(tile_c)::value;
+        constexpr int S0 = (Q + 1) & 3, S1 = (Q + 2) & 3, S2 = (Q + 3) & 3;      // ring positions of the planes p, p+1, p+2 (= p-2)
+        constexpr int QM1 = (Q + 3) & 3, QM2 = (Q + 2) & 3;                      // B planes / own B of p-1, p-2
+        T(&x1)[3] = xh[Q & 1];
+        const T(&xp)[3] = xh[(Q + 1) & 1];
+        T(&Bp)[3] = Bh[Q];
         // ---------------- A(p): push-forward of the plane p at the own node ----------------
-        T Bp[3] = { T(0), T(0), T(0) };
-        if (TILE || (has_node && p >= k0 && p < kend)) {
-            T dF[3][3];
-            const T* fr = f1 + ox;
+        const bool work = TILE || (has_node && p < kend);
+        const T* fr = px + S0 * L::SLOTX;
+        T dF[3][3], bq[3];
+        if (work) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 x1[c] = fr[c * CSX];
                 dF[c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
                 dF[c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
+                bq[c] = pb[S0 * L::SLOTB + c * CSB];
             }
-            if (p == 0) {                   // bottom face: -3 x(0) + 4 x(1) - x(2)
-                const T* f3 = sx + s2 * L::SLOTX;
+        } else if (!TILE && has_node) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) dF[c][2] = T(4) * f2[ox + c * CSX] - T(3) * x1[c] - f3[ox + c * CSX];
-            } else if (p + 1 <= nz - 1) {
+            for (int c = 0; c < 3; ++c) x1[c] = fr[c * CSX];
+        }
+        ptx::mbar_wait(bar_x + 8u * S1, Q >= 2 ? gpar ^ 1u : gpar);             // the plane p+1
+        if (work) {
+            const T* f2 = px + S1 * L::SLOTX;
 #pragma unroll
-                for (int c = 0; c < 3; ++c) dF[c][2] = f2[ox + c * CSX] - xc[c];
-            } else {                        // top face: 3 x(nz-1) - 4 x(nz-2) + x(nz-3); plane nz-3 is still in its slot
-                const T* fm = sx + sm2 * L::SLOTX;
+            for (int c = 0; c < 3; ++c) dF[c][2] = f2[c * CSX] - xp[c];
+            const unsigned special = edge | (p == 0 ? 16u : 0u) | (p == nz - 1 ? 32u : 0u);
+            if (special) {
+                if (special & 16u) {            // bottom face: -3 x(0) + 4 x(1) - x(2)
+                    const T* f3 = px + S2 * L::SLOTX;
 #pragma unroll
-                for (int c = 0; c < 3; ++c) dF[c][2] = T(3) * x1[c] - T(4) * xc[c] + fm[ox + c * CSX];
+                    for (int c = 0; c < 3; ++c) dF[c][2] = T(4) * f2[c * CSX] - T(3) * x1[c] - f3[c * CSX];
+                }
+                if (special & 32u) {            // top face: 3 x(nz-1) - 4 x(nz-2) + x(nz-3); the plane nz-3 is still in its position
+                    const T* fm = px + S2 * L::SLOTX;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) dF[c][2] = T(3) * x1[c] - T(4) * xp[c] + fm[c * CSX];
+                }
+                if (special & 15u) face_fix<T, BW, CSX>(fr, special & 15u, dF);
             }
-            if (edge) face_fix<T, BW, CSX>(fr, edge, dF);
-            T n0[3], inv;
-            duo_push<T, CSB>(dF, bs + ob, twoh, n0, Bp, inv, ok, dom);
-            T* d = sB + buf * L::BSLOT + oB;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) dF[c][c] += twoh[c];
+            T n0[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+                n0[c] = dF[c1][1] * dF[c2][2] - dF[c2][1] * dF[c1][2];
+            }
+            const T D = dF[0][0] * n0[0] + dF[1][0] * n0[1] + dF[2][0] * n0[2];
+            ok = ok && (positive_finite(D) || !dom);
+            const T inv = fast_rcp(D);
+            // dF b first, the division last: the nine products do not wait for the reciprocal's Newton chain
+#pragma unroll
+            for (int c = 0; c < 3; ++c) Bp[c] = (dF[c][0] * bq[0] + dF[c][1] * bq[1] + dF[c][2] * bq[2]) * inv;
+            T* d = pB + Q * L::BSLOT;
             d[0] = Bp[0];
             d[BCS] = Bp[1];
             d[2 * BCS] = Bp[2];
             if constexpr (TILE) {
-                const T sn = (p > 0 && p < nz - 1 && in_xy) ? a.dtg * inv : T(0);
-                uint32_t w0[CW], w1[CW];
+                sh[Q & 1] = (p > 0 && p < nz - 1 && in_xy) ? a.dtg * inv : T(0);
+                uint32_t w0[C0W], w1[C1W];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    W32::put(w0 + c * W32::N, dF[c][0]);
-                    W32::put(w0 + (3 + c) * W32::N, dF[c][1]);
-                    W32::put(w1 + c * W32::N, dF[c][2]);
-                    W32::put(w1 + (3 + c) * W32::N, n0[c]);
+                    W32::put(w0 + c * WN, dF[c][0]);
+                    W32::put(w0 + (3 + c) * WN, dF[c][1]);
+                    W32::put(w1 + c * WN, dF[c][2]);
                 }
-                W32::put(w0 + 6 * W32::N, x1[0]);
-                W32::put(w0 + 7 * W32::N, x1[1]);
-                W32::put(w1 + 6 * W32::N, sn);
-                W32::put(w1 + 7 * W32::N, x1[2]);
-                const uint32_t ra = tm0 + rp * REC;
-                if constexpr (CW == 16) { tmem::st16(ra, w0); tmem::st16(ra + CW, w1); }
-                else { tmem::st8(ra, w0); tmem::st8(ra + CW, w1); }
+                W32::put(w0 + 6 * WN, n0[0]);
+                W32::put(w0 + 7 * WN, n0[1]);
+                W32::put(w1 + 3 * WN, n0[2]);
+                tmem::st<C0W>(tm0 + (Q & 1) * REC, w0);
+                tmem::st<C1W>(tm0 + (Q & 1) * REC + C0W, w1);
             }
-        } else if (!TILE && has_node) {
-            const T* fr = f1 + ox;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) x1[c] = fr[c * CSX];
         }
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(bar_full + 8u * (uint32_t)buf);      // this warp's part of B(p) is in shared memory
+        if (lane == 0) ptx::mbar_arrive(bar_full + 8u * Q);         // this warp's part of B(p) is in shared memory
         if (!TILE && pwarp) {
-            ptx::named_sync(BAR_A + buf, NW * 32);            // every warp is done with the xi / b planes p
-            if (producer) refill(p + R);
+            ptx::named_sync(BAR_A + Q, NW * 32);                    // every warp is done with the xi / b planes p
+            if (producer) refill(p + L::R);
         } else {
-            ptx::named_arrive(BAR_A + buf, NW * 32);
+            ptx::named_arrive(BAR_A + Q, NW * 32);
         }
         // ---------------- F(p-1): finish the plane t = p-1 ----------------
+        // (every warp waits for FULL[p-1]: that keeps the ring warps, too, from overwriting a B plane still in use; a
+        // chunk that starts inside the grid runs F(k0 - 1) once without storing it: the plane belongs to the chunk below)
         if (p > first_p) {
-            ptx::mbar_wait(bar_full + 8u * (uint32_t)pb, ppar);   // every warp has published B(p-1) (about an iteration ago)
-            const int t = p - 1;
-            if (TILE && t >= k0) {
-                uint32_t w0[CW], w1[CW];
-                const uint32_t ra = tm0 + (rp ^ 1u) * REC;
-                if constexpr (CW == 16) { tmem::ld16(ra, w0); tmem::ld16(ra + CW, w1); }
-                else { tmem::ld8(ra, w0); tmem::ld8(ra + CW, w1); }
-                const T* g = sB + pb * L::BSLOT + oB;
+            uint32_t w0[C0W], w1[C1W];
+            if constexpr (TILE) {
+                tmem::wait_st();                                     // record(p-1) was stored an iteration ago
+                tmem::ld<C0W>(tm0 + ((Q + 1) & 1) * REC, w0);
+                tmem::ld<C1W>(tm0 + ((Q + 1) & 1) * REC + C0W, w1);
+            }
+            ptx::mbar_wait(bar_full + 8u * QM1, Q == 0 ? gpar ^ 1u : gpar);     // every warp has published B(p-1)
+            if constexpr (TILE) {
+                const T* g = pB + QM1 * L::BSLOT;
+                const T(&Bc)[3] = Bh[QM1];
+                const T(&Bm)[3] = Bh[QM2];
                 T dBi[3], dBj[3], dBk[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -224,69 +282,116 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 }
                 tmem::wait_ld(w0);
                 tmem::wait_ld(w1);
-                T c0[3], c1[3], c2[3], n0[3], n1[3], n2[3], x[3], DJ[3], uu[3];
+                T c0[3], c1[3], c2[3], n0[3], n1[3], n2[3], DJ[3], uu[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    c0[c] = W32::get(w0 + c * W32::N);
-                    c1[c] = W32::get(w0 + (3 + c) * W32::N);
-                    c2[c] = W32::get(w1 + c * W32::N);
-                    n0[c] = W32::get(w1 + (3 + c) * W32::N);
+                    c0[c] = W32::get(w0 + c * WN);
+                    c1[c] = W32::get(w0 + (3 + c) * WN);
+                    c2[c] = W32::get(w1 + c * WN);
                 }
-                x[0] = W32::get(w0 + 6 * W32::N);
-                x[1] = W32::get(w0 + 7 * W32::N);
-                x[2] = W32::get(w1 + 7 * W32::N);
-                const T s = W32::get(w1 + 6 * W32::N);
+                n0[0] = W32::get(w0 + 6 * WN);
+                n0[1] = W32::get(w0 + 7 * WN);
+                n0[2] = W32::get(w1 + 3 * WN);
                 cross_set(c2, c0, n1);                  // n_1 = dF_2 x dF_0,  n_2 = dF_0 x dF_1  (Eqs. 2.5/2.6)
                 cross_set(c0, c1, n2);
                 cross_set(n0, dBi, DJ);
                 cross_acc(n1, dBj, DJ);
                 cross_acc(n2, dBk, DJ);
                 cross_set(DJ, Bc, uu);
+                if constexpr (DIAG) {
+                    if (p > k0) diag_node(p - 1, c0, n0, Bc, uu);
+                } else {
+                    const T s = sh[(Q + 1) & 1];
+                    T x[3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], x[c]);
-                ok = ok && is_finite(x[0] + x[1] + x[2]);
-                if (st) {
-                    po[0] = x[0];
-                    po[a.comp] = x[1];
-                    po[2 * a.comp] = x[2];
+                    for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], xp[c]);
+                    ok = ok && is_finite(x[0] + x[1] + x[2]);
+                    if (st && p > k0) {
+                        po[0] = x[0];
+                        po[a.comp] = x[1];
+                        po[2 * a.comp] = x[2];
+                    }
+                    po += a.plane;
                 }
-                po += a.plane;
             }
         }
+    };
+    auto run = [&](auto tile_c) {
+#pragma unroll 1
+        for (;;) {
+            body(Phase<0>{}, tile_c);
+            if (++p > kend) break;
+            body(Phase<1>{}, tile_c);
+            if (++p > kend) break;
+            body(Phase<2>{}, tile_c);
+            if (++p > kend) break;
+            body(Phase<3>{}, tile_c);
+            if (++p > kend) break;
+            gpar ^= 1u;
+        }
+    };
+    if (tilew) run(std::true_type{});
+    else run(std::false_type{});
+
+    if (k1 == nz && tilew) {   // the top plane (line-tied) is carried through / enters the energy sum
+        const int ql = (nz - 1 - first_p) & 3;
+        if constexpr (DIAG) {
+            uint32_t w0[C0W], w1[C1W];
+            tmem::wait_st();                                // (tcgen05 operations are warp-wide: no per-thread predicate here)
+            tmem::ld<C0W>(tm0 + (ql & 1) * REC, w0);
+            tmem::ld<C1W>(tm0 + (ql & 1) * REC + C0W, w1);
+            tmem::wait_ld(w0);
+            tmem::wait_ld(w1);
+            T c0[3], n0[3], Bt[3];
+            const T zero[3] = { T(0), T(0), T(0) };
 #pragma unroll
-        for (int c = 0; c < 3; ++c) { Bm[c] = Bc[c]; Bc[c] = Bp[c]; xc[c] = x1[c]; }
-        if constexpr (TILE) tmem::wait_st();                  // record(p) is complete before the next iteration reads it
-        pb = buf; ppar = cpar;
-        if (++buf == NB) { buf = 0; cpar ^= 1u; }
-        rp ^= 1u;
-        sm2 = sm1; sm1 = s0; s0 = s1; s1 = s2;
-        if (s1 == 0) par1 ^= 1u;
-        if (++s2 == R) s2 = 0;
-    }
-  };
-  if (tilew) run(std::true_type{});
-  else run(std::false_type{});
-    if (k1 == nz && st) {   // the top plane (line-tied) is carried through
-        T* pl = out + (long long)(nz - 1) * a.plane + (long long)gj * a.pitch + gi;
-        pl[0] = x1[0];
-        pl[a.comp] = x1[1];
-        pl[2 * a.comp] = x1[2];
+            for (int c = 0; c < 3; ++c) {
+                c0[c] = W32::get(w0 + c * WN);
+                Bt[c] = ql == 0 ? Bh[0][c] : ql == 1 ? Bh[1][c] : ql == 2 ? Bh[2][c] : Bh[3][c];
+            }
+            n0[0] = W32::get(w0 + 6 * WN);
+            n0[1] = W32::get(w0 + 7 * WN);
+            n0[2] = W32::get(w1 + 3 * WN);
+            diag_node(nz - 1, c0, n0, Bt, zero);
+        } else if (st) {
+            T* pl = out + (long long)(nz - 1) * a.plane + (long long)gj * a.pitch + gi;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) pl[c * a.comp] = (ql & 1) ? xh[1][c] : xh[0][c];
+        }
     }
     if (!ok) atomicOr(a.flag, FLAG_NUMERIC);
     tmem::fence_before_sync();
-    __syncthreads();
-    if (warp == 0) tmem::dealloc<512>(tm_base_s);
+    __syncthreads();                                        // the pipeline is drained: shared memory is free
+    if constexpr (DIAG) {
+        // fixed-order reduction: lanes by a shuffle tree, then the tile warps in index order; one partial per CTA
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            DiagPartial w;
+            w.e = __shfl_down_sync(0xffffffffu, acc.e, o);
+            w.fmax = __shfl_down_sync(0xffffffffu, acc.fmax, o);
+            w.xi = __shfl_down_sync(0xffffffffu, acc.xi, o);
+            w.dmin = __shfl_down_sync(0xffffffffu, acc.dmin, o);
+            diag_combine(acc, w);
+        }
+        DiagPartial* shp = reinterpret_cast<DiagPartial*>(smem);
+        if (tilew && lane == 0) shp[warp] = acc;
+        __syncthreads();
+        if (tid == 0) {
+            DiagPartial v = shp[0];
+            for (int w = 1; w < NTW; ++w) diag_combine(v, shp[w]);
+            reinterpret_cast<DiagPartial*>(out)[blockIdx.x] = v;
+        }
+    }
+    if (warp == 0) tmem::dealloc<L::TMEM_COLS>(tm_base_s);
 }
 
 // ----------------------------------------------------------------------------------------------- host side
 
-constexpr int kSTY = 16, kSR = 4, kSRB = 4, kSNB = 4;
-
 inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* xi0, void* xi1, void* b, int sm_count,
                            std::string* why)
 {
-    using Ld = SymLayout<double, kSTY, kSR, kSRB, kSNB>;
-    using Lf = SymLayout<float, kSTY, kSR, kSRB, kSNB>;
+    using Ld = SymLayout<double>;
+    using Lf = SymLayout<float>;
     p->usable = false;
     p->f64 = f64;
     p->g = g;
@@ -295,16 +400,23 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
     p->b = b;
     p->name = f64 ? "sym_tmem_f64" : "sym_tmem_f32";
     const int bw = f64 ? Ld::BW : Lf::BW;
-    if (!encode_map(&p->map_xi[0], f64, xi0, g, bw, kSTY + 4) || !encode_map(&p->map_xi[1], f64, xi1, g, bw, kSTY + 4) ||
-        !encode_map(&p->map_b, f64, b, g, bw, kSTY + 2)) {
+    if (!encode_map(&p->map_xi[0], f64, xi0, g, bw, Ld::TY + 4) || !encode_map(&p->map_xi[1], f64, xi1, g, bw, Ld::TY + 4) ||
+        !encode_map(&p->map_b, f64, b, g, bw, Ld::TY + 2)) {
         *why = "cuTensorMapEncodeTiled failed";
         return false;
     }
     p->tiles_x = (g.nx + Ld::TX - 1) / Ld::TX;
-    p->tiles_y = (g.ny + kSTY - 1) / kSTY;
+    p->tiles_y = (g.ny + Ld::TY - 1) / Ld::TY;
     p->smem_bytes = f64 ? Ld::BYTES : Lf::BYTES;
-    cudaError_t e = f64 ? cudaFuncSetAttribute(k_step_sym<double, kSTY, kSR, kSRB, kSNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes)
-                        : cudaFuncSetAttribute(k_step_sym<float, kSTY, kSR, kSRB, kSNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes);
+    cudaError_t e = cudaSuccess;
+    const int sb = (int)p->smem_bytes;
+    if (f64) {
+        e = cudaFuncSetAttribute(k_step_sym<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+    } else {
+        e = cudaFuncSetAttribute(k_step_sym<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+    }
     if (e != cudaSuccess) {
         *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
         return false;
@@ -315,9 +427,8 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
 }
 
 template <typename T>
-inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream)
+inline StreamArgs<T> sym_args(const StreamPlan& p, T dtg, int* flag)
 {
-    using L = SymLayout<T, kSTY, kSR, kSRB, kSNB>;
     StreamArgs<T> a;
     a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
     a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
@@ -327,8 +438,26 @@ inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* fla
     a.ntiles = p.tiles_x * p.tiles_y;
     a.chunk_len = p.chunk_len;
     a.flag = flag;
-    const int grid = a.ntiles * p.nchunks;
-    k_step_sym<T, kSTY, kSR, kSRB, kSNB><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, static_cast<T*>(p.xi[1 - cur]), a);
+    return a;
+}
+
+template <typename T>
+inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream)
+{
+    const StreamArgs<T> a = sym_args<T>(p, dtg, flag);
+    k_step_sym<T, false><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
+                                                                                                  static_cast<T*>(p.xi[1 - cur]), a);
+    return cudaGetLastError();
+}
+
+// S6 of the state in buffer `cur` by the same pass (no update, no store): one DiagPartial per CTA into `partials`
+template <typename T>
+inline cudaError_t launch_sym_diag(const StreamPlan& p, int cur, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
+{
+    const StreamArgs<T> a = sym_args<T>(p, (T)0, flag);
+    *nblocks = a.ntiles * p.nchunks;
+    k_step_sym<T, true><<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
+                                                                                    reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();
 }
 

@@ -46,6 +46,10 @@ __device__ __forceinline__ void st8(uint32_t taddr, const uint32_t (&r)[8])
     asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
                  "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]));
 }
+__device__ __forceinline__ void st4(uint32_t taddr, const uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]));
+}
 // asynchronous loads: the registers are valid only after wait_ld over the same registers
 __device__ __forceinline__ void ld16(uint32_t taddr, uint32_t (&r)[16])
 {
@@ -60,6 +64,10 @@ __device__ __forceinline__ void ld8(uint32_t taddr, uint32_t (&r)[8])
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
                  : "r"(taddr));
 }
+__device__ __forceinline__ void ld4(uint32_t taddr, uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr));
+}
 // Wait for every earlier tcgen05.ld of this thread.  The registers go through the statement as in/out operands so
 // that the compiler cannot move a use of them above the wait.
 __device__ __forceinline__ void wait_ld(uint32_t (&r)[16])
@@ -72,6 +80,19 @@ __device__ __forceinline__ void wait_ld(uint32_t (&r)[8])
 {
     asm volatile("tcgen05.wait::ld.sync.aligned;"
                  : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]));
+}
+__device__ __forceinline__ void wait_ld(uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]));
+}
+// N = 16 / 8 / 4 words by one operation
+template <int N> __device__ __forceinline__ void st(uint32_t taddr, const uint32_t (&r)[N])
+{
+    if constexpr (N == 16) st16(taddr, r); else if constexpr (N == 8) st8(taddr, r); else st4(taddr, r);
+}
+template <int N> __device__ __forceinline__ void ld(uint32_t taddr, uint32_t (&r)[N])
+{
+    if constexpr (N == 16) ld16(taddr, r); else if constexpr (N == 8) ld8(taddr, r); else ld4(taddr, r);
 }
 
 // One value per operation: a double is its own aligned register pair, so that no register has to be moved into a
