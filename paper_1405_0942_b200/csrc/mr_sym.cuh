@@ -4,15 +4,19 @@
 // Work item = (32 x 16 xy tile, chunk of z-planes); a CTA marches along k.  Per plane the TMA unit streams the box of
 // xi (halo 2 in j, 16 bytes in i) and of b (halo 1) into one of four shared-memory ring positions.  Each of the 16
 // tile warps owns one row of the tile (one node per thread); four more warps own the halo-1 ring of the tile (row
-// below, row above, both columns; only B is formed there) and the TMA producer.  In iteration p a tile warp does
+// below, row above, both columns; only B is formed there) and the TMA producer.  Iteration p of a tile warp:
 //     A(p):    dF, n_0 = dF_1 x dF_2, D = dF_0 . n_0, 1/D, B(p) = dF b / D (Eq. 2.1) -> shared B plane p % 4;
-//              record(p) = (dF, n_0) -> Tensor Memory (own columns);  mbarrier.arrive FULL[p % 4]
-//     F(p-1):  wait FULL[(p-1) % 4] -- a phase that completed about one iteration ago --,
-//              D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x (B(p) - B(p-2))   (closed form of Eqs. 2.3-2.7),
-//              u = gamma J x B (Eq. 1.5), xi+ = xi + dt u -> HBM          (DIAG: the reduction of S6 instead).
-// The two halves belong to different planes and are independent: every warp carries the same load and nobody waits
-// for the slowest warp of the current plane.  A warp that starts A(p) has seen FULL[p-2] complete, i.e. every warp has
-// finished F(p-4): four B planes suffice.
+//              record(p) = (dF, n_0) -> Tensor Memory (own columns);
+//     arrive READY[p] (one lane), bar.arrive SLOT[p];  wait READY[p-1]
+//     F(p-1):  record(p-1) <- Tensor Memory;  D J = n_0 x delta_i B + n_1 x delta_j B + n_2 x (B(p) - B(p-2))  (closed
+//              form of Eqs. 2.3-2.7), u = gamma J x B (Eq. 1.5), xi+ = xi + dt u -> HBM   (DIAG: the reduction of S6).
+// One mbarrier phase READY[t] = "every warp has published B(t)" AND "the plane t+3 has landed": the TMA of the plane
+// t+3 completes its bytes on that barrier, so a warp polls ONE barrier per plane, half an iteration after the phase
+// it waits for began to fill (the wait is a poll, not a stall), and A(p+1) starts without any wait.  A(p) and F(p-1)
+// belong to different planes and are independent: every warp carries the same load and nobody waits for the slowest
+// warp of the current plane.  A warp that starts A(p) has seen READY[p-2] complete, i.e. every warp has finished
+// F(p-4): four B planes suffice.  The producer's warp collects the bar.arrive of SLOT[p] (every warp is done with the
+// xi / b planes p) and requests the plane p+4 into that ring position.
 //
 // The k loop is unrolled by four with the phase q = (p - first_p) % 4 a compile-time constant: every ring position,
 // B plane, barrier, TMEM record and the rotating register sets (own B of the last planes: period 4, own xi: period 2)
@@ -46,7 +50,7 @@ struct SymLayout {
     static constexpr size_t OFF_B0 = OFF_X + (size_t)R * SLOTX * sizeof(T);
     static constexpr size_t OFF_BB = OFF_B0 + (size_t)R * SLOTB * sizeof(T);
     static constexpr size_t OFF_BAR = OFF_BB + (size_t)NB * BSLOT * sizeof(T);
-    static constexpr size_t BYTES = OFF_BAR + (size_t)(R + NB) * 8 + 128;
+    static constexpr size_t BYTES = OFF_BAR + (size_t)NB * 8 + 128;
     // TMEM record of a node: chunk 0 = columns 0, 1 of dF, n_0[0], n_0[1] (8 values), chunk 1 = column 2 of dF, n_0[2]
     static constexpr int WN = (int)sizeof(T) / 4;                   // 32-bit words per value
     static constexpr int C0W = 8 * WN, C1W = 4 * WN, REC = 16 * WN; // record stride (12 values, padded to 16)
@@ -57,15 +61,15 @@ template <int Q> using Phase = std::integral_constant<int, Q>;
 
 template <typename T, bool DIAG>
 __global__ void __maxnreg__(96)
-k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, T* __restrict__ out,
-           const StreamArgs<T> a)
+k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, const T* __restrict__ in,
+           T* __restrict__ out, const StreamArgs<T> a)
 {
     using L = SymLayout<T>;
     using W32 = tmem::Words<T>;
     constexpr int TX = L::TX, TY = L::TY, NTW = L::NTW, BW = L::BW, CSX = L::CSX, CSB = L::CSB, BBW = L::BBW, BCS = L::BCS;
     constexpr int NW = L::NWARPS, WN = L::WN, C0W = L::C0W, C1W = L::C1W, REC = L::REC;
     static_assert(L::TMEM_COLS == 256 || L::TMEM_COLS == 128, "TMEM columns: a power of two");
-    constexpr int BAR_A = 1;                                        // named barriers BAR_A .. BAR_A + 3
+    constexpr uint32_t PLANE_BYTES = L::XBOX_BYTES + L::BBOX_BYTES;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t tm_base_s;
     unsigned char* smem = smem_raw + ((128u - (ptx::smem_u32(smem_raw) & 127u)) & 127u);
@@ -73,7 +77,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const T* sb = reinterpret_cast<const T*>(smem + L::OFF_B0);
     T* sB = reinterpret_cast<T*>(smem + L::OFF_BB);
     const uint32_t sx_u32 = ptx::smem_u32(sx), sb_u32 = ptx::smem_u32(sb);
-    const uint32_t bar_x = ptx::smem_u32(smem + L::OFF_BAR), bar_full = bar_x + 8u * L::R;
+    const uint32_t bar = ptx::smem_u32(smem + L::OFF_BAR);          // READY[0..3]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool tilew = warp < NTW;
@@ -83,13 +87,12 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int k0 = chunk * a.chunk_len, k1 = min(k0 + a.chunk_len, nz);
     const int kend = min(k1, nz - 1);               // planes k0 .. kend-1 are finished here (and nz-1 carried through)
     const int first_p = max(k0 - 1, 0);             // B is formed on the planes first_p .. kend
-    const int pfirst = max(first_p - 1, 0), plast = min(kend + 1, nz - 1);       // xi / b planes this item touches
+    const int plast = min(kend + 1, nz - 1);        // last xi / b plane this item touches
     const T twoh[3] = { a.twoh[0], a.twoh[1], a.twoh[2] };
 
     const bool pwarp = warp == NW - 1, producer = pwarp && lane == 0;
     if (producer) {
-        for (int s = 0; s < L::R; ++s) ptx::mbar_init(bar_x + 8u * s, 1);
-        for (int s = 0; s < L::NB; ++s) ptx::mbar_init(bar_full + 8u * s, NW);   // one arrival per warp
+        for (int s = 0; s < 4; ++s) ptx::mbar_init(bar + 8u * s, NW);           // one arrival per working warp + the producer's
         ptx::fence_mbar_init();
     }
     if (warp == 0) tmem::alloc<L::TMEM_COLS>(&tm_base_s);
@@ -98,25 +101,32 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     tmem::fence_after_sync();
     const uint32_t tm0 = tm_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 2 * REC);
 
-    // Ring position of the plane p: (p - first_p + 1) % 4, one mbarrier per position for the xi box and the b box (they
-    // are born and die together).  The plane nz does not exist: it is "delivered" empty, so that the consumers wait for
-    // the plane p+1 unconditionally.
-    int next_x = pfirst;
-    auto refill = [&](int upto) {
-        for (; next_x <= upto; ++next_x) {
-            const uint32_t s = (uint32_t)(next_x - first_p + 1) & 3u;
-            if (next_x <= plast) {
-                ptx::mbar_expect_tx(bar_x + 8u * s, L::XBOX_BYTES + L::BBOX_BYTES);
-                ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, next_x, 0, bar_x + 8u * s);
-                ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, next_x, 0, bar_x + 8u * s);
-            } else if (next_x == nz) {
-                ptx::mbar_arrive(bar_x + 8u * s);
-            }
+    // The plane P = first_p + r lives in the ring position (r + 1) % 4 and completes its bytes on READY[(r + 1) % 4] in
+    // the phase of the plane t = P - 3.  A plane beyond the item's last one is "delivered" empty: the producer's arrival alone.
+    constexpr int BAR_SLOT = 1;                       // named barriers BAR_SLOT .. BAR_SLOT + 3
+    auto request = [&](int r) {                       // producer: the plane first_p + r
+        const uint32_t s = (uint32_t)(r + 1) & 3u, b = bar + 8u * s;
+        const int P = first_p + r;
+        if (P <= plast) {
+            ptx::mbar_expect_tx(b, PLANE_BYTES);
+            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, P, 0, b);
+            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, P, 0, b);
+        } else {
+            ptx::mbar_arrive(b);
         }
     };
-    if (producer) {
-        if (first_p == 0) ptx::mbar_arrive(bar_x);          // position 0 would hold the plane -1: its first phase is empty
-        refill(pfirst + 3);
+    if (pwarp) {
+        if (producer)
+            for (int r = 0; r < 4; ++r) request(r);
+        // the producer's warp: SLOT[p] complete = every warp is done with the xi / b planes p -> the plane p + 4
+        for (int u = 0; first_p + u <= kend; ++u) {
+            ptx::named_sync(BAR_SLOT + (u & 3), NW * 32);
+            if (producer) request(u + 4);
+        }
+    } else {
+        // the phases of the planes first_p - 3 .. first_p - 1 publish no B: the working warps arrive right away
+        __syncwarp();
+        if (lane == 0) { ptx::mbar_arrive(bar + 8u); ptx::mbar_arrive(bar + 16u); ptx::mbar_arrive(bar + 24u); }
     }
 
     // the node of this thread: tile warps own the row `warp` of the tile; ring warps a node of the halo-1 ring (row below,
@@ -137,20 +147,18 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const bool in_xy = gi > 0 && gi < a.nx - 1 && gj > 0 && gj < a.ny - 1;
     const bool st = tilew && dom;
 
-    // the planes first_p - 1 (own xi for the first k-difference), first_p and, for the one-sided difference on the bottom
-    // face, 2
-    if (first_p > 0) ptx::mbar_wait(bar_x, 0u);
-    ptx::mbar_wait(bar_x + 8u, 0u);
-    if (first_p == 0) ptx::mbar_wait(bar_x + 24u, 0u);
-
     bool ok = true;
     T xh[2][3], Bh[4][3], sh[2];                             // own xi(p), xi(p-1); own B(p) .. B(p-3); dt gamma / D of p, p-1
+    {
+        // own xi of the plane below the first one (for the first k-difference) straight from global memory
+        const long long o = (long long)(first_p - 1) * a.plane + (long long)gj * a.pitch + gi;
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        xh[0][c] = T(0);
-        xh[1][c] = first_p > 0 ? px[c * CSX] : T(0);        // phase 0 reads xi(first_p - 1) from xh[1]
+        for (int c = 0; c < 3; ++c) {
+            xh[0][c] = T(0);
+            xh[1][c] = (first_p > 0 && dom) ? in[c * a.comp + o] : T(0);        // phase 0 reads xi(first_p - 1) from xh[1]
 #pragma unroll
-        for (int q = 0; q < 4; ++q) Bh[q][c] = T(0);
+            for (int q = 0; q < 4; ++q) Bh[q][c] = T(0);
+        }
     }
     sh[0] = sh[1] = T(0);
     T* po = out + (long long)first_p * a.plane + (long long)gj * a.pitch + gi;     // plane t = p-1 of the first F
@@ -170,6 +178,11 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         diag_combine(acc, v);
     };
 
+    if (!pwarp) {        // the planes first_p, first_p + 1 and, for the one-sided difference on the bottom face, 2
+        ptx::mbar_wait(bar + 8u, 0u);
+        ptx::mbar_wait(bar + 16u, 0u);
+        if (first_p == 0) ptx::mbar_wait(bar + 24u, 0u);
+    }
     int p = first_p;
     uint32_t gpar = 0u;                                      // parity of the group of four planes
     auto body = [&](auto phase, auto tile_c) {
@@ -180,27 +193,21 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         T(&x1)[3] = xh[Q & 1];
         const T(&xp)[3] = xh[(Q + 1) & 1];
         T(&Bp)[3] = Bh[Q];
+        const bool fin = TILE && p > first_p;
         // ---------------- A(p): push-forward of the plane p at the own node ----------------
         const bool work = TILE || (has_node && p < kend);
         const T* fr = px + S0 * L::SLOTX;
-        T dF[3][3], bq[3];
         if (work) {
+            const T* f2 = px + S1 * L::SLOTX;
+            T dF[3][3], bq[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 x1[c] = fr[c * CSX];
                 dF[c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
                 dF[c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
+                dF[c][2] = f2[c * CSX] - xp[c];
                 bq[c] = pb[S0 * L::SLOTB + c * CSB];
             }
-        } else if (!TILE && has_node) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) x1[c] = fr[c * CSX];
-        }
-        ptx::mbar_wait(bar_x + 8u * S1, Q >= 2 ? gpar ^ 1u : gpar);             // the plane p+1
-        if (work) {
-            const T* f2 = px + S1 * L::SLOTX;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) dF[c][2] = f2[c * CSX] - xp[c];
             const unsigned special = edge | (p == 0 ? 16u : 0u) | (p == nz - 1 ? 32u : 0u);
             if (special) {
                 if (special & 16u) {            // bottom face: -3 x(0) + 4 x(1) - x(2)
@@ -235,84 +242,77 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             d[2 * BCS] = Bp[2];
             if constexpr (TILE) {
                 sh[Q & 1] = (p > 0 && p < nz - 1 && in_xy) ? a.dtg * inv : T(0);
-                uint32_t w0[C0W], w1[C1W];
+                uint32_t v0[C0W], v1[C1W];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    W32::put(w0 + c * WN, dF[c][0]);
-                    W32::put(w0 + (3 + c) * WN, dF[c][1]);
-                    W32::put(w1 + c * WN, dF[c][2]);
+                    W32::put(v0 + c * WN, dF[c][0]);
+                    W32::put(v0 + (3 + c) * WN, dF[c][1]);
+                    W32::put(v1 + c * WN, dF[c][2]);
                 }
-                W32::put(w0 + 6 * WN, n0[0]);
-                W32::put(w0 + 7 * WN, n0[1]);
-                W32::put(w1 + 3 * WN, n0[2]);
-                tmem::st<C0W>(tm0 + (Q & 1) * REC, w0);
-                tmem::st<C1W>(tm0 + (Q & 1) * REC + C0W, w1);
+                W32::put(v0 + 6 * WN, n0[0]);
+                W32::put(v0 + 7 * WN, n0[1]);
+                W32::put(v1 + 3 * WN, n0[2]);
+                tmem::st<C0W>(tm0 + (Q & 1) * REC, v0);
+                tmem::st<C1W>(tm0 + (Q & 1) * REC + C0W, v1);
             }
+        } else if (!TILE && has_node) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) x1[c] = fr[c * CSX];
         }
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(bar_full + 8u * Q);         // this warp's part of B(p) is in shared memory
-        if (!TILE && pwarp) {
-            ptx::named_sync(BAR_A + Q, NW * 32);                    // every warp is done with the xi / b planes p
-            if (producer) refill(p + L::R);
-        } else {
-            ptx::named_arrive(BAR_A + Q, NW * 32);
-        }
+        if (lane == 0) ptx::mbar_arrive(bar + 8u * Q);                   // this warp's part of B(p) is in shared memory
+        ptx::named_arrive(BAR_SLOT + Q, NW * 32);                        // ... and it is done with the xi / b planes p
+        ptx::mbar_wait(bar + 8u * QM1, Q >= 2 ? gpar ^ 1u : gpar);      // B(p-1) is published, the plane p+2 has landed
         // ---------------- F(p-1): finish the plane t = p-1 ----------------
-        // (every warp waits for FULL[p-1]: that keeps the ring warps, too, from overwriting a B plane still in use; a
-        // chunk that starts inside the grid runs F(k0 - 1) once without storing it: the plane belongs to the chunk below)
-        if (p > first_p) {
+        // (a chunk that starts inside the grid runs F(k0 - 1) once without storing it: the plane belongs to the chunk below)
+        if (fin) {
             uint32_t w0[C0W], w1[C1W];
-            if constexpr (TILE) {
-                tmem::wait_st();                                     // record(p-1) was stored an iteration ago
-                tmem::ld<C0W>(tm0 + ((Q + 1) & 1) * REC, w0);
-                tmem::ld<C1W>(tm0 + ((Q + 1) & 1) * REC + C0W, w1);
+            tmem::wait_st();                                 // record(p-1) was stored an iteration ago
+            tmem::ld<C0W>(tm0 + ((Q + 1) & 1) * REC, w0);
+            tmem::ld<C1W>(tm0 + ((Q + 1) & 1) * REC + C0W, w1);
+            const T* g = pB + QM1 * L::BSLOT;
+            const T(&Bc)[3] = Bh[QM1];
+            const T(&Bm)[3] = Bh[QM2];
+            T dBi[3], dBj[3], dBk[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const T* gc = g + c * BCS;
+                dBi[c] = gc[1] - gc[-1];
+                dBj[c] = gc[BBW] - gc[-BBW];
+                dBk[c] = Bp[c] - Bm[c];
             }
-            ptx::mbar_wait(bar_full + 8u * QM1, Q == 0 ? gpar ^ 1u : gpar);     // every warp has published B(p-1)
-            if constexpr (TILE) {
-                const T* g = pB + QM1 * L::BSLOT;
-                const T(&Bc)[3] = Bh[QM1];
-                const T(&Bm)[3] = Bh[QM2];
-                T dBi[3], dBj[3], dBk[3];
+            tmem::wait_ld(w0);
+            tmem::wait_ld(w1);
+            T c0[3], c1[3], c2[3], n0[3], n1[3], n2[3], DJ[3], uu[3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const T* gc = g + c * BCS;
-                    dBi[c] = gc[1] - gc[-1];
-                    dBj[c] = gc[BBW] - gc[-BBW];
-                    dBk[c] = Bp[c] - Bm[c];
-                }
-                tmem::wait_ld(w0);
-                tmem::wait_ld(w1);
-                T c0[3], c1[3], c2[3], n0[3], n1[3], n2[3], DJ[3], uu[3];
+            for (int c = 0; c < 3; ++c) {
+                c0[c] = W32::get(w0 + c * WN);
+                c1[c] = W32::get(w0 + (3 + c) * WN);
+                c2[c] = W32::get(w1 + c * WN);
+            }
+            n0[0] = W32::get(w0 + 6 * WN);
+            n0[1] = W32::get(w0 + 7 * WN);
+            n0[2] = W32::get(w1 + 3 * WN);
+            cross_set(c2, c0, n1);                  // n_1 = dF_2 x dF_0,  n_2 = dF_0 x dF_1  (Eqs. 2.5/2.6)
+            cross_set(c0, c1, n2);
+            cross_set(n0, dBi, DJ);
+            cross_acc(n1, dBj, DJ);
+            cross_acc(n2, dBk, DJ);
+            cross_set(DJ, Bc, uu);
+            if constexpr (DIAG) {
+                if (p > k0) diag_node(p - 1, c0, n0, Bc, uu);
+            } else {
+                const T s = sh[(Q + 1) & 1];
+                T x[3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    c0[c] = W32::get(w0 + c * WN);
-                    c1[c] = W32::get(w0 + (3 + c) * WN);
-                    c2[c] = W32::get(w1 + c * WN);
+                for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], xp[c]);
+                ok = ok && is_finite(x[0] + x[1] + x[2]);
+                if (st && p > k0) {
+                    po[0] = x[0];
+                    po[a.comp] = x[1];
+                    po[2 * a.comp] = x[2];
                 }
-                n0[0] = W32::get(w0 + 6 * WN);
-                n0[1] = W32::get(w0 + 7 * WN);
-                n0[2] = W32::get(w1 + 3 * WN);
-                cross_set(c2, c0, n1);                  // n_1 = dF_2 x dF_0,  n_2 = dF_0 x dF_1  (Eqs. 2.5/2.6)
-                cross_set(c0, c1, n2);
-                cross_set(n0, dBi, DJ);
-                cross_acc(n1, dBj, DJ);
-                cross_acc(n2, dBk, DJ);
-                cross_set(DJ, Bc, uu);
-                if constexpr (DIAG) {
-                    if (p > k0) diag_node(p - 1, c0, n0, Bc, uu);
-                } else {
-                    const T s = sh[(Q + 1) & 1];
-                    T x[3];
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], xp[c]);
-                    ok = ok && is_finite(x[0] + x[1] + x[2]);
-                    if (st && p > k0) {
-                        po[0] = x[0];
-                        po[a.comp] = x[1];
-                        po[2 * a.comp] = x[2];
-                    }
-                    po += a.plane;
-                }
+                po += a.plane;
             }
         }
     };
@@ -331,7 +331,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         }
     };
     if (tilew) run(std::true_type{});
-    else run(std::false_type{});
+    else if (!pwarp) run(std::false_type{});
 
     if (k1 == nz && tilew) {   // the top plane (line-tied) is carried through / enters the energy sum
         const int ql = (nz - 1 - first_p) & 3;
@@ -445,8 +445,8 @@ template <typename T>
 inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream)
 {
     const StreamArgs<T> a = sym_args<T>(p, dtg, flag);
-    k_step_sym<T, false><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
-                                                                                                  static_cast<T*>(p.xi[1 - cur]), a);
+    k_step_sym<T, false><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+        p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), static_cast<T*>(p.xi[1 - cur]), a);
     return cudaGetLastError();
 }
 
@@ -456,8 +456,8 @@ inline cudaError_t launch_sym_diag(const StreamPlan& p, int cur, DiagPartial* pa
 {
     const StreamArgs<T> a = sym_args<T>(p, (T)0, flag);
     *nblocks = a.ntiles * p.nchunks;
-    k_step_sym<T, true><<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b,
-                                                                                    reinterpret_cast<T*>(partials), a);
+    k_step_sym<T, true><<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+        p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();
 }
 
