@@ -53,7 +53,11 @@ struct SymLayout {
     static constexpr size_t BYTES = OFF_BAR + (size_t)NB * 8 + 128;
     // TMEM record of a node: chunk 0 = columns 0, 1 of dF, n_0[0], n_0[1] (8 values), chunk 1 = column 2 of dF, n_0[2]
     static constexpr int WN = (int)sizeof(T) / 4;                   // 32-bit words per value
+    #ifdef MR_X_TMEM
+    static constexpr int C0W = 8 * WN, C1W = 8 * WN, REC = 16 * WN; // + own xi (3 values) in chunk 1
+#else
     static constexpr int C0W = 8 * WN, C1W = 4 * WN, REC = 16 * WN; // record stride (12 values, padded to 16)
+#endif
     static constexpr int TMEM_COLS = (NTW / 4) * 2 * REC;           // warps of a lane quarter x two records (plane parity)
 };
 
@@ -161,6 +165,12 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         }
     }
     sh[0] = sh[1] = T(0);
+#ifndef MR_BM_REG
+    if (tilew) {         // the first F reads the own B of the plane first_p - 1 (never formed) from the B plane 3: a finite stand-in
+#pragma unroll
+        for (int c = 0; c < 3; ++c) pB[3 * L::BSLOT + c * BCS] = T(0);
+    }
+#endif
     T* po = out + (long long)first_p * a.plane + (long long)gj * a.pitch + gi;     // plane t = p-1 of the first F
     DiagPartial acc = { 0.0, 0.0, 0.0, INFINITY };          // DIAG: this thread's partial
     const double zxy = ((gi == 0 || gi == a.nx - 1) ? 0.5 : 1.0) * ((gj == 0 || gj == a.ny - 1) ? 0.5 : 1.0);   // Eq. 3.13
@@ -183,6 +193,9 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         ptx::mbar_wait(bar + 16u, 0u);
         if (first_p == 0) ptx::mbar_wait(bar + 24u, 0u);
     }
+#ifdef MR_STAGGER
+    if (tilew && (warp & 1)) __nanosleep(MR_STAGGER);
+#endif
     int p = first_p;
     uint32_t gpar = 0u;                                      // parity of the group of four planes
     auto body = [&](auto phase, auto tile_c) {
@@ -252,6 +265,12 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 W32::put(v0 + 6 * WN, n0[0]);
                 W32::put(v0 + 7 * WN, n0[1]);
                 W32::put(v1 + 3 * WN, n0[2]);
+#ifdef MR_X_TMEM
+                W32::put(v1 + 4 * WN, x1[0]);
+                W32::put(v1 + 5 * WN, x1[1]);
+                W32::put(v1 + 6 * WN, x1[2]);
+                W32::put(v1 + 7 * WN, T(0));
+#endif
                 tmem::st<C0W>(tm0 + (Q & 1) * REC, v0);
                 tmem::st<C1W>(tm0 + (Q & 1) * REC + C0W, v1);
             }
@@ -271,8 +290,18 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             tmem::ld<C0W>(tm0 + ((Q + 1) & 1) * REC, w0);
             tmem::ld<C1W>(tm0 + ((Q + 1) & 1) * REC + C0W, w1);
             const T* g = pB + QM1 * L::BSLOT;
+#ifdef MR_BC_SMEM
+            const T Bc[3] = { g[0], g[BCS], g[2 * BCS] };
+#else
             const T(&Bc)[3] = Bh[QM1];
+#endif
+#ifndef MR_BM_REG
+            // own B(p-2) back from its shared plane (intact until A(p+2)): cheaper than six more registers carried
+            const T* gm = pB + QM2 * L::BSLOT;
+            const T Bm[3] = { gm[0], gm[BCS], gm[2 * BCS] };
+#else
             const T(&Bm)[3] = Bh[QM2];
+#endif
             T dBi[3], dBj[3], dBk[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
@@ -305,8 +334,14 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 const T s = sh[(Q + 1) & 1];
                 T x[3];
 #pragma unroll
+#ifdef MR_X_TMEM
+                for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], W32::get(w1 + (4 + c) * WN));
+#else
                 for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], xp[c]);
+#endif
+#ifndef MR_NOXCHK
                 ok = ok && is_finite(x[0] + x[1] + x[2]);
+#endif
                 if (st && p > k0) {
                     po[0] = x[0];
                     po[a.comp] = x[1];
