@@ -24,6 +24,17 @@
  *   Q5  time stepping on this path is forward Euler with all u from the old x;
  *   Q8  line-tied on all six faces: boundary nodes never move, J and u are 0 there;
  *   Q9  xi = max over interior nodes of the pointwise ratio |JxB|/|B|^2.
+ *   Q12 periodic axis (Eqs. 2.12-2.14, :147-164): every node of the axis is an inner point, the ghost nodes are
+ *       x(f-1) = x(l) - (L + dX) e_a and x(l+1) = x(f) + (L + dX) e_a with L = X_l - X_f, i.e. the period is n_a h_a;
+ *       B(X,0) is periodic;
+ *   Q22 integrator (section 2.4, :131-143): Cash-Karp RK5(4), the step advances with the fifth-order solution,
+ *       Lambda = max over nodes and components of |x5 - x4|; reject if Lambda > Lambda0 and retry with Eq. 2.11;
+ *       accept otherwise, and enlarge dt by Eq. 2.11 if Lambda < Lambda0/2 (growth capped at 5x: Lambda may be 0);
+ *       the last step is clipped to end at t_end without changing the dt handed on;
+ *   Q23 convexity (Eqs. 3.10-3.11, :231-243): kappa(node) = 1 iff every trihedron of the node whose three
+ *       neighbours exist has sgn det = di dj dk, else -1;
+ *   Q24 eps* (Eq. 3.7, :214): alpha* = J.B/B^2 at the interior nodes of the grid line through (i_c, j_c), maximum
+ *       over ordered pairs of a_r (alpha*_i - alpha*_j)/|X_i - X_j|.
  *
  * Return codes: 0 ok, 1 bad argument, 5 numeric failure (det <= 0, non-finite, or singular normal matrix).
  */
@@ -57,7 +68,14 @@ typedef struct {
     size_t N;
     double h[3];
     double lo[3];
+    int per[3];    /* 1 = periodic axis (Eqs. 2.12-2.14), 0 = line-tied faces */
+    double P[3];   /* period n_a h_a = L_a + dX_a (reading Q12) */
 } grid_t;
+
+/* Boundary type per logical axis for every call that follows: 0 line-tied (default), 1 periodic.  A process-wide
+ * setting (the oracle is single-user test infrastructure); the Python wrapper sets it around each call. */
+static int g_bc[3] = { 0, 0, 0 };
+void mro_set_bc(const int bc[3]) { for (int a = 0; a < 3; ++a) g_bc[a] = bc ? (bc[a] != 0) : 0; }
 
 static int make_grid(const int n[3], const double lo[3], const double hi[3], grid_t* g)
 {
@@ -72,6 +90,8 @@ static int make_grid(const int n[3], const double lo[3], const double hi[3], gri
         } else {
             g->h[a] = 1.0; g->lo[a] = 0.0;
         }
+        g->per[a] = g_bc[a];
+        g->P[a] = (double)n[a] * g->h[a];
     }
     return MRO_OK;
 }
@@ -79,6 +99,27 @@ static int make_grid(const int n[3], const double lo[3], const double hi[3], gri
 static inline size_t at(const grid_t* g, int i, int j, int k)
 {
     return ((size_t)k * (size_t)g->ny + (size_t)j) * (size_t)g->nx + (size_t)i;
+}
+
+/* Value of one component f of a nodal field at an index that may lie one or two nodes outside a PERIODIC axis: the
+ * index is wrapped (B is periodic, Eq. 2.14); if f is the component `shift` of the positions x, the ghost value is
+ * shifted by -/+ (L + dX) along that axis (Eqs. 2.12, 2.13).  shift = -1 for periodic fields. */
+static double val(const grid_t* g, const double* f, int shift, int i, int j, int k)
+{
+    int idx[3] = { i, j, k };
+    const int n[3] = { g->nx, g->ny, g->nz };
+    double add = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        if (idx[a] < 0) { idx[a] += n[a]; if (a == shift) add -= g->P[a]; }
+        else if (idx[a] >= n[a]) { idx[a] -= n[a]; if (a == shift) add += g->P[a]; }
+    }
+    return f[at(g, idx[0], idx[1], idx[2])] + add;
+}
+
+/* is the node an inner point along every axis (line-tied faces excluded, periodic axes have no faces)? */
+static int inner_node(const grid_t* g, int i, int j, int k)
+{
+    return (g->per[0] || (i > 0 && i < g->nx - 1)) && (g->per[1] || (j > 0 && j < g->ny - 1)) && (g->per[2] || (k > 0 && k < g->nz - 1));
 }
 
 /* X_ijk, the fixed reference grid ("x(X,0)=X"; :170 rectangular grid). */
@@ -97,9 +138,14 @@ int mro_reference_grid(const int n[3], const double lo[3], const double hi[3], d
 }
 
 /* ---- O1: first derivative of a nodal scalar along logical axis a at node (i,j,k) (reading Q3) ---------- */
-static double ddX(const grid_t* g, const double* f, int a, int i, int j, int k)
+static double ddX(const grid_t* g, const double* f, int a, int i, int j, int k, int shift)
 {
     int idx[3] = { i, j, k };
+    if (g->per[a]) {              /* periodic axis: central everywhere, ghosts by Eqs. 2.12-2.14 */
+        int p[3] = { i, j, k }, m[3] = { i, j, k };
+        p[a] += 1; m[a] -= 1;
+        return (val(g, f, shift, p[0], p[1], p[2]) - val(g, f, shift, m[0], m[1], m[2])) / (2.0 * g->h[a]);
+    }
     int na = (a == 0) ? g->nx : (a == 1) ? g->ny : g->nz;
     int c = idx[a];
     int p1[3] = { i, j, k }, p2[3] = { i, j, k };
@@ -127,7 +173,7 @@ static void jacobian_at(const grid_t* g, const double* x, int i, int j, int k, d
 {
     for (int c = 0; c < 3; ++c)
         for (int a = 0; a < 3; ++a)
-            F[c][a] = ddX(g, x + (size_t)c * g->N, a, i, j, k);
+            F[c][a] = ddX(g, x + (size_t)c * g->N, a, i, j, k, c);
 }
 
 /* O1+O2 on all nodes: F[(c*3+a)*N + p] = dx_c/dX_a, det[p] = Delta.  F or det may be NULL. */
@@ -212,6 +258,15 @@ static void load3(const grid_t* g, const double* f, int i, int j, int k, double 
     size_t p = at(g, i, j, k);
     v[0] = f[p]; v[1] = f[g->N + p]; v[2] = f[2 * g->N + p];
 }
+/* neighbour values across a periodic face: positions (shifted ghost, Eqs. 2.12/2.13) and periodic fields (Eq. 2.14) */
+static void load3x(const grid_t* g, const double* x, int i, int j, int k, double v[3])
+{
+    for (int c = 0; c < 3; ++c) v[c] = val(g, x + (size_t)c * g->N, c, i, j, k);
+}
+static void load3f(const grid_t* g, const double* f, int i, int j, int k, double v[3])
+{
+    for (int c = 0; c < 3; ++c) v[c] = val(g, f + (size_t)c * g->N, -1, i, j, k);
+}
 
 /*
  * O4m at one interior node: the nearest-neighbour mimetic curl, literally.
@@ -234,8 +289,8 @@ static int curl_mimetic_at(const grid_t* g, const double* x, const double* B, in
         off[0][a] = +1; off[1][b] = +1; off[2][a] = -1; off[3][b] = -1;
         double xr[4][3], Br[4][3];
         for (int r = 0; r < 4; ++r) {
-            load3(g, x, i + off[r][0], j + off[r][1], k + off[r][2], xr[r]);
-            load3(g, B, i + off[r][0], j + off[r][1], k + off[r][2], Br[r]);
+            load3x(g, x, i + off[r][0], j + off[r][1], k + off[r][2], xr[r]);
+            load3f(g, B, i + off[r][0], j + off[r][1], k + off[r][2], Br[r]);
         }
         double circ = 0.0, nA[3] = { 0.0, 0.0, 0.0 };
         for (int r = 0; r < 4; ++r) {
@@ -260,16 +315,19 @@ static int curl_mimetic_at(const grid_t* g, const double* x, const double* B, in
 }
 
 /* O4m on the grid: J at interior nodes from GIVEN nodal x and B; J = 0 on boundary nodes (reading Q8). */
-int mro_curl_mimetic(const int n[3], const double* x, const double* B, double* J)
+/* (lo/hi may be NULL when no axis is periodic: the operator itself does not use the spacing, only the period does) */
+int mro_curl_mimetic_dom(const int n[3], const double lo[3], const double hi[3], const double* x, const double* B, double* J)
 {
-    grid_t g; int rc = make_grid(n, NULL, NULL, &g); if (rc) return rc;
+    grid_t g; int rc = make_grid(n, lo, hi, &g); if (rc) return rc;
+    if ((!lo || !hi) && (g.per[0] || g.per[1] || g.per[2])) return MRO_BADARG;
     int bad = 0;
     memset(J, 0, 3 * g.N * sizeof(double));
 #pragma omp parallel for num_threads(g_threads) reduction(| : bad)
-    for (int k = 1; k < g.nz - 1; ++k)
-        for (int j = 1; j < g.ny - 1; ++j)
-            for (int i = 1; i < g.nx - 1; ++i) {
+    for (int k = 0; k < g.nz; ++k)
+        for (int j = 0; j < g.ny; ++j)
+            for (int i = 0; i < g.nx; ++i) {
                 double Jl[3];
+                if (!inner_node(&g, i, j, k)) continue;
                 if (curl_mimetic_at(&g, x, B, i, j, k, Jl)) { bad = 1; continue; }
                 size_t p = at(&g, i, j, k);
                 for (int c = 0; c < 3; ++c) J[(size_t)c * g.N + p] = Jl[c];
@@ -277,21 +335,27 @@ int mro_curl_mimetic(const int n[3], const double* x, const double* B, double* J
     return bad ? MRO_NUMERIC : MRO_OK;
 }
 
+int mro_curl_mimetic(const int n[3], const double* x, const double* B, double* J)
+{
+    return mro_curl_mimetic_dom(n, NULL, NULL, x, B, J);
+}
+
 /* second derivative d2 f / dX_a dX_b at an interior node (compact central differences, reading Q4) */
-static double d2dX(const grid_t* g, const double* f, int a, int b, int i, int j, int k)
+static double d2dX(const grid_t* g, const double* f, int a, int b, int i, int j, int k, int shift)
 {
     int o[3] = { i, j, k };
     if (a == b) {
         int p[3] = { i, j, k }, m[3] = { i, j, k };
         p[a] += 1; m[a] -= 1;
-        return (f[at(g, p[0], p[1], p[2])] - 2.0 * f[at(g, o[0], o[1], o[2])] + f[at(g, m[0], m[1], m[2])]) / (g->h[a] * g->h[a]);
+        return (val(g, f, shift, p[0], p[1], p[2]) - 2.0 * f[at(g, o[0], o[1], o[2])] + val(g, f, shift, m[0], m[1], m[2])) / (g->h[a] * g->h[a]);
     }
     int pp[3] = { i, j, k }, pm[3] = { i, j, k }, mp[3] = { i, j, k }, mm[3] = { i, j, k };
     pp[a] += 1; pp[b] += 1;
     pm[a] += 1; pm[b] -= 1;
     mp[a] -= 1; mp[b] += 1;
     mm[a] -= 1; mm[b] -= 1;
-    return (f[at(g, pp[0], pp[1], pp[2])] - f[at(g, pm[0], pm[1], pm[2])] - f[at(g, mp[0], mp[1], mp[2])] + f[at(g, mm[0], mm[1], mm[2])])
+    return (val(g, f, shift, pp[0], pp[1], pp[2]) - val(g, f, shift, pm[0], pm[1], pm[2]) - val(g, f, shift, mp[0], mp[1], mp[2])
+            + val(g, f, shift, mm[0], mm[1], mm[2]))
            / (4.0 * g->h[a] * g->h[b]);
 }
 
@@ -327,10 +391,10 @@ static int curl_direct_at(const grid_t* g, const double* x, const double* B0, in
     for (int c = 0; c < 3; ++c)
         for (int a = 0; a < 3; ++a)
             for (int b = 0; b < 3; ++b)
-                H[c][a][b] = d2dX(g, x + (size_t)c * g->N, a, b, i, j, k);
+                H[c][a][b] = d2dX(g, x + (size_t)c * g->N, a, b, i, j, k, c);
     for (int c = 0; c < 3; ++c)
         for (int a = 0; a < 3; ++a)
-            G[c][a] = ddX(g, B0 + (size_t)c * g->N, a, i, j, k);
+            G[c][a] = ddX(g, B0 + (size_t)c * g->N, a, i, j, k, -1);
     load3(g, B0, i, j, k, b0);
 
     double Nv[3], dN[3][3], dD[3], dB[3][3], dBdx[3][3];
@@ -372,10 +436,11 @@ int mro_curl_direct(const int n[3], const double lo[3], const double hi[3], cons
     int bad = 0;
     memset(J, 0, 3 * g.N * sizeof(double));
 #pragma omp parallel for num_threads(g_threads) reduction(| : bad)
-    for (int k = 1; k < g.nz - 1; ++k)
-        for (int j = 1; j < g.ny - 1; ++j)
-            for (int i = 1; i < g.nx - 1; ++i) {
+    for (int k = 0; k < g.nz; ++k)
+        for (int j = 0; j < g.ny; ++j)
+            for (int i = 0; i < g.nx; ++i) {
                 double Jl[3];
+                if (!inner_node(&g, i, j, k)) continue;
                 if (curl_direct_at(&g, x, B0, i, j, k, Jl)) { bad = 1; continue; }
                 size_t p = at(&g, i, j, k);
                 for (int c = 0; c < 3; ++c) J[(size_t)c * g.N + p] = Jl[c];
@@ -397,7 +462,7 @@ int mro_fields(const int n[3], const double lo[3], const double hi[3], const dou
     double* Jl = J ? J : (double*)malloc(3 * g.N * sizeof(double));
     if (!Bl || !Jl) return MRO_BADARG;
     rc = mro_push_forward(n, lo, hi, x, B0, Bl, det);
-    int rc2 = (op == 0) ? mro_curl_mimetic(n, x, Bl, Jl) : mro_curl_direct(n, lo, hi, x, B0, Jl);
+    int rc2 = (op == 0) ? mro_curl_mimetic_dom(n, lo, hi, x, Bl, Jl) : mro_curl_direct(n, lo, hi, x, B0, Jl);
     if (u) {
         /* J is 0 on boundary nodes, hence u = 0 there (line-tied, :147) */
 #pragma omp parallel for num_threads(g_threads)
@@ -456,12 +521,12 @@ int mro_diagnostics(const int n[3], const double lo[3], const double hi[3], cons
                 double b[3] = { B[p], B[g.N + p], B[2 * g.N + p] };
                 double b2 = b[0] * b[0] + b[1] * b[1] + b[2] * b[2];
                 double zeta = 1.0;
-                if (i == 0 || i == g.nx - 1) zeta *= 0.5;
-                if (j == 0 || j == g.ny - 1) zeta *= 0.5;
-                if (k == 0 || k == g.nz - 1) zeta *= 0.5;
+                if (!g.per[0] && (i == 0 || i == g.nx - 1)) zeta *= 0.5;
+                if (!g.per[1] && (j == 0 || j == g.ny - 1)) zeta *= 0.5;
+                if (!g.per[2] && (k == 0 || k == g.nz - 1)) zeta *= 0.5;
                 E += (long double)(zeta * b2 * det[p]);
                 if (det[p] < dmin || isnan(det[p])) dmin = det[p];
-                int interior = i > 0 && i < g.nx - 1 && j > 0 && j < g.ny - 1 && k > 0 && k < g.nz - 1;
+                int interior = inner_node(&g, i, j, k);
                 if (interior) {
                     double jv[3] = { J[p], J[g.N + p], J[2 * g.N + p] }, f[3];
                     cross3(jv, b, f);
@@ -473,5 +538,231 @@ int mro_diagnostics(const int n[3], const double lo[3], const double hi[3], cons
     out[0] = (double)(0.5L * E * (long double)g.h[0] * (long double)g.h[1] * (long double)g.h[2]);
     out[1] = fmax; out[2] = xi; out[3] = dmin;
     free(B); free(J); free(det);
+    return rc;
+}
+
+/* =========================================================================================================
+ * Time stepping of section 2.4: the fifth-order adaptive Runge-Kutta formula of Cash & Karp
+ * ([4] of the paper) with the embedded fourth-order solution, step control by Eq. 2.11 (reading Q22).
+ * ========================================================================================================= */
+
+/* Butcher tableau of the Cash-Karp pair (Cash & Karp 1990; also Press et al., the paper's [21]). */
+static const double CK_A[6][5] = {
+    { 0.0, 0.0, 0.0, 0.0, 0.0 },
+    { 1.0 / 5.0, 0.0, 0.0, 0.0, 0.0 },
+    { 3.0 / 40.0, 9.0 / 40.0, 0.0, 0.0, 0.0 },
+    { 3.0 / 10.0, -9.0 / 10.0, 6.0 / 5.0, 0.0, 0.0 },
+    { -11.0 / 54.0, 5.0 / 2.0, -70.0 / 27.0, 35.0 / 27.0, 0.0 },
+    { 1631.0 / 55296.0, 175.0 / 512.0, 575.0 / 13824.0, 44275.0 / 110592.0, 253.0 / 4096.0 } };
+static const double CK_B5[6] = { 37.0 / 378.0, 0.0, 250.0 / 621.0, 125.0 / 594.0, 0.0, 512.0 / 1771.0 };
+static const double CK_B4[6] = { 2825.0 / 27648.0, 0.0, 18575.0 / 48384.0, 13525.0 / 55296.0, 277.0 / 14336.0, 1.0 / 4.0 };
+
+/* right-hand side of an autonomous system y' = f(y) with m unknowns; returns 0 or an error code */
+typedef int (*mro_rhs_fn)(const double* y, double* dydt, void* user);
+
+/*
+ * One trial step of size dt from y (m values): y5 = fifth-order, y4 = embedded fourth-order solution (either may
+ * be NULL), *lambda = max_q |y5_q - y4_q| (the "maximum error").  Stage s evaluates f at
+ * y + dt sum_{r<s} a_sr k_r; work must hold 7 m doubles.  Plain loops in the order of the tableau.
+ */
+int mro_cash_karp_trial(long long m, const double* y, double dt, mro_rhs_fn f, void* user, double* y5, double* y4,
+                        double* lambda, double* work)
+{
+    double* k[6];
+    for (int s = 0; s < 6; ++s) k[s] = work + (size_t)s * (size_t)m;
+    double* ys = work + (size_t)6 * (size_t)m;
+    for (int s = 0; s < 6; ++s) {
+        for (long long q = 0; q < m; ++q) {
+            double acc = 0.0;
+            for (int r = 0; r < s; ++r) acc += CK_A[s][r] * k[r][q];
+            ys[q] = y[q] + dt * acc;
+        }
+        int rc = f(ys, k[s], user);
+        if (rc) return rc;
+    }
+    double lam = 0.0;
+    for (long long q = 0; q < m; ++q) {
+        double s5 = 0.0, s4 = 0.0;
+        for (int s = 0; s < 6; ++s) { s5 += CK_B5[s] * k[s][q]; s4 += CK_B4[s] * k[s][q]; }
+        double v5 = y[q] + dt * s5, v4 = y[q] + dt * s4;
+        double e = fabs(v5 - v4);
+        if (e > lam || isnan(e)) lam = e;
+        if (y5) y5[q] = v5;
+        if (y4) y4[q] = v4;
+    }
+    *lambda = lam;
+    return MRO_OK;
+}
+
+/*
+ * Step control of PAPER.md:139-143: returns 1 if the trial step is accepted (Lambda <= Lambda0), 0 if it is
+ * rejected, and writes the step length to use next: Eq. 2.11 dt' = dt |Lambda0/Lambda|^0.2 after a rejection or
+ * when Lambda < Lambda0/2 (growth capped at 5 dt, Lambda may vanish), dt otherwise.
+ */
+int mro_step_control(double dt, double lambda, double lambda0, double* dt_next)
+{
+    if (lambda > lambda0 || isnan(lambda)) {
+        *dt_next = isnan(lambda) ? 0.5 * dt : dt * pow(fabs(lambda0 / lambda), 0.2);
+        return 0;
+    }
+    if (lambda < 0.5 * lambda0) {
+        double f = lambda > 0.0 ? pow(fabs(lambda0 / lambda), 0.2) : 5.0;
+        *dt_next = dt * (f > 5.0 ? 5.0 : f);
+    } else {
+        *dt_next = dt;
+    }
+    return 1;
+}
+
+typedef struct {
+    const int* n; const double* lo; const double* hi; const double* B0; double gamma; int op;
+} relax_rhs_t;
+
+static int relax_rhs(const double* x, double* u, void* user)
+{
+    const relax_rhs_t* r = (const relax_rhs_t*)user;
+    return mro_fields(r->n, r->lo, r->hi, x, r->B0, r->gamma, r->op, NULL, NULL, u, NULL);
+}
+
+/*
+ * Integrate dx/dt = u(x) = gamma J x B (Eq. 1.5) from *t to t_end with the adaptive Cash-Karp scheme.
+ * *dt: first trial step in, step handed on out.  trace (may be NULL, capacity trace_cap rows of 4 doubles) records every
+ * trial: {t, dt tried, Lambda, accepted}.  counts[0] = accepted, counts[1] = rejected trials.
+ * Returns 0, 1 (bad argument), 5 (numeric failure; x holds the last accepted state) or 7 (max_trials exhausted).
+ */
+int mro_step_adaptive(const int n[3], const double lo[3], const double hi[3], double* x, const double* B0, double gamma,
+                      int op, double t_end, double lambda0, double* t, double* dt, long long max_trials,
+                      long long counts[2], double* trace, long long trace_cap)
+{
+    grid_t g; int rc = make_grid(n, lo, hi, &g); if (rc) return rc;
+    if (!(lambda0 > 0.0) || !(*dt > 0.0) || !t || !dt || !counts) return MRO_BADARG;
+    const long long m = (long long)(3 * g.N);
+    double* work = (double*)malloc((size_t)8 * (size_t)m * sizeof(double));
+    if (!work) return MRO_BADARG;
+    double* y5 = work + (size_t)7 * (size_t)m;
+    relax_rhs_t r = { n, lo, hi, B0, gamma, op };
+    counts[0] = counts[1] = 0;
+    long long trials = 0;
+    rc = MRO_OK;
+    while (*t < t_end) {
+        if (trials >= max_trials) { rc = 7; break; }
+        const double rest = t_end - *t;
+        const int clipped = *dt >= rest;
+        const double h = clipped ? rest : *dt;
+        double lam = 0.0, dt_next = 0.0;
+        rc = mro_cash_karp_trial(m, x, h, relax_rhs, &r, y5, NULL, &lam, work);
+        if (rc) break;
+        const int ok = mro_step_control(h, lam, lambda0, &dt_next);
+        if (trace && trials < trace_cap) {
+            trace[4 * trials + 0] = *t; trace[4 * trials + 1] = h; trace[4 * trials + 2] = lam; trace[4 * trials + 3] = (double)ok;
+        }
+        ++trials;
+        if (ok) {
+            memcpy(x, y5, (size_t)m * sizeof(double));
+            *t = clipped ? t_end : *t + h;
+            counts[0]++;
+            if (!clipped || dt_next < *dt) *dt = dt_next;      /* a clipped last step does not change the dt handed on */
+        } else {
+            counts[1]++;
+            *dt = dt_next;
+        }
+    }
+    free(work);
+    return rc;
+}
+
+/* =========================================================================================================
+ * Diagnostics of section 3.2 beyond E_M and xi: convexity (Eqs. 3.10-3.11), alpha* and eps* (Eqs. 3.5-3.7),
+ * sigma_B and sigma_x (Eqs. 3.8-3.9).
+ * ========================================================================================================= */
+
+/* kappa per node (int, +1 / -1; reading Q23) and the number of nodes with kappa = -1.  kappa may be NULL. */
+int mro_convexity(const int n[3], const double lo[3], const double hi[3], const double* x, int* kappa, long long* n_concave)
+{
+    grid_t g; int rc = make_grid(n, lo, hi, &g); if (rc) return rc;
+    const int nn[3] = { g.nx, g.ny, g.nz };
+    long long bad = 0;
+    for (int k = 0; k < g.nz; ++k)
+        for (int j = 0; j < g.ny; ++j)
+            for (int i = 0; i < g.nx; ++i) {
+                const int idx[3] = { i, j, k };
+                double xc[3]; load3(&g, x, i, j, k, xc);
+                int kap = 1;
+                for (int di = -1; di <= 1; di += 2)
+                    for (int dj = -1; dj <= 1; dj += 2)
+                        for (int dk = -1; dk <= 1; dk += 2) {
+                            const int d[3] = { di, dj, dk };
+                            int exists = 1;
+                            for (int a = 0; a < 3; ++a)
+                                if (!g.per[a] && (idx[a] + d[a] < 0 || idx[a] + d[a] >= nn[a])) exists = 0;
+                            if (!exists) continue;
+                            double v[3][3], nb[3];   /* v[0] = dx^lambda, v[1] = dx^mu, v[2] = dx^nu (Eq. 3.10) */
+                            load3x(&g, x, i + di, j, k, nb); for (int c = 0; c < 3; ++c) v[0][c] = nb[c] - xc[c];
+                            load3x(&g, x, i, j + dj, k, nb); for (int c = 0; c < 3; ++c) v[1][c] = nb[c] - xc[c];
+                            load3x(&g, x, i, j, k + dk, nb); for (int c = 0; c < 3; ++c) v[2][c] = nb[c] - xc[c];
+                            const double dd = det3(v);    /* det of the matrix with rows dx^lambda, dx^mu, dx^nu */
+                            const int sgn = dd > 0.0 ? 1 : (dd < 0.0 ? -1 : 0);
+                            if (sgn != di * dj * dk) kap = -1;           /* Eq. 3.11 */
+                        }
+                if (kappa) kappa[at(&g, i, j, k)] = kap;
+                if (kap < 0) ++bad;
+            }
+    if (n_concave) *n_concave = bad;
+    return MRO_OK;
+}
+
+/*
+ * alpha* = J.B/B^2 (Eq. 3.5) at the inner nodes of the grid line (ic, jc, .) -- s_alpha of Eq. 3.6 when that line is the
+ * z axis -- into alpha[nz] (0 at line-tied end nodes), and eps* = max over ordered pairs (k1, k2), k1 != k2, of
+ * a_r (alpha*_k1 - alpha*_k2)/|X_k1 - X_k2| (Eq. 3.7; reference positions X).  alpha may be NULL.
+ */
+int mro_eps_star(const int n[3], const double lo[3], const double hi[3], const double* x, const double* B0, int op,
+                 int ic, int jc, double a_r, double* alpha, double* eps)
+{
+    grid_t g; int rc = make_grid(n, lo, hi, &g); if (rc) return rc;
+    if (ic < 0 || ic >= g.nx || jc < 0 || jc >= g.ny || !inner_node(&g, ic, jc, g.nz / 2)) return MRO_BADARG;
+    double* B = (double*)malloc(3 * g.N * sizeof(double));
+    double* J = (double*)malloc(3 * g.N * sizeof(double));
+    double* al = (double*)malloc((size_t)g.nz * sizeof(double));
+    if (!B || !J || !al) return MRO_BADARG;
+    rc = mro_fields(n, lo, hi, x, B0, 1.0, op, B, J, NULL, NULL);
+    const int k_lo = g.per[2] ? 0 : 1, k_hi = g.per[2] ? g.nz - 1 : g.nz - 2;
+    for (int k = 0; k < g.nz; ++k) {
+        size_t p = at(&g, ic, jc, k);
+        double b[3] = { B[p], B[g.N + p], B[2 * g.N + p] }, jv[3] = { J[p], J[g.N + p], J[2 * g.N + p] };
+        al[k] = (k >= k_lo && k <= k_hi) ? (jv[0] * b[0] + jv[1] * b[1] + jv[2] * b[2]) / (b[0] * b[0] + b[1] * b[1] + b[2] * b[2]) : 0.0;
+        if (alpha) alpha[k] = al[k];
+    }
+    double e = 0.0;
+    for (int k1 = k_lo; k1 <= k_hi; ++k1)
+        for (int k2 = k_lo; k2 <= k_hi; ++k2) {
+            if (k1 == k2) continue;
+            double s = a_r * (al[k1] - al[k2]) / fabs((double)(k1 - k2) * g.h[2]);
+            if (s > e) e = s;
+        }
+    *eps = e;
+    free(B); free(J); free(al);
+    return rc;
+}
+
+/* sigma_B (Eq. 3.8) and sigma_x (Eq. 3.9): root of the mean over ALL N nodes of |B - B_ref|^2 resp. |x - x_ref|^2. */
+int mro_sigma(const int n[3], const double lo[3], const double hi[3], const double* x, const double* B0,
+              const double* x_ref, const double* B_ref, double* sigma_x, double* sigma_B)
+{
+    grid_t g; int rc = make_grid(n, lo, hi, &g); if (rc) return rc;
+    double* B = (double*)malloc(3 * g.N * sizeof(double));
+    if (!B) return MRO_BADARG;
+    rc = mro_push_forward(n, lo, hi, x, B0, B, NULL);
+    long double sx = 0.0L, sb = 0.0L;
+    for (size_t p = 0; p < g.N; ++p)
+        for (int c = 0; c < 3; ++c) {
+            double dx = x[(size_t)c * g.N + p] - x_ref[(size_t)c * g.N + p];
+            double db = B[(size_t)c * g.N + p] - B_ref[(size_t)c * g.N + p];
+            sx += (long double)(dx * dx);
+            sb += (long double)(db * db);
+        }
+    *sigma_x = sqrt((double)(sx / (long double)g.N));
+    *sigma_B = sqrt((double)(sb / (long double)g.N));
+    free(B);
     return rc;
 }
