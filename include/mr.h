@@ -18,8 +18,10 @@
  *   - Ownership: the CALLER owns every device and host buffer and the stream.  The library never allocates
  *     device memory: mr_create binds a caller-provided workspace of at least mr_workspace_bytes() bytes
  *     (256-byte aligned) that must outlive the context.  mr_ctx itself is host memory owned by the library.
- *   - All work is enqueued on the caller's stream.  mr_step, mr_diagnostics and the *_host calls synchronise
- *     that stream before returning; mr_set_B0, mr_set_x and mr_get_fields are asynchronous.
+ *   - All work is enqueued on the caller's stream.  mr_set_B0, mr_get_fields, mr_get_xi and mr_rhs are asynchronous
+ *     (the buffers may be reused once the stream has passed the call); every other call synchronises that stream
+ *     before it returns (mr_set_x / mr_set_xi for the check of the line-tied faces, mr_step* for the error flag, the
+ *     diagnostics for their scalars, the *_host calls for the copies).
  *   - Errors are return codes; nothing throws or aborts.  mr_last_error(ctx) gives a message for the last
  *     failing call on that context.  After MR_ERR_NUMERIC the context stays failed until mr_set_x succeeds.
  */
@@ -51,7 +53,9 @@ typedef enum {
 
 typedef enum {
     MR_BC_LINE_TIED = 0, /* u = 0 and B.n fixed on the face (:147) */
-    MR_BC_PERIODIC = 1   /* Eqs. 2.12-2.14; NOT IMPLEMENTED: mr_create returns MR_ERR_INVALID_ARG */
+    MR_BC_PERIODIC = 1   /* Eqs. 2.12-2.14 (:147-164): every node of the axis is an inner point, nodes at lo + idx*h,
+                            period n*h = (hi - lo) + h; the ghost nodes are x(-1) = x(n-1) - n*h e_a, x(n) = x(0) + n*h e_a
+                            and B(X,0) must be periodic.  Runs on the global-memory kernels (csrc/mr_generic.cuh). */
 } mr_bc;
 
 typedef enum { MR_F64 = 0, MR_F32 = 1 } mr_dtype;
@@ -61,7 +65,7 @@ typedef struct { double lo[3], hi[3]; } mr_domain;   /* hi > lo componentwise */
 
 /* "boundary" + options of mr_create */
 typedef struct {
-    mr_bc bc[3];            /* per logical axis (both faces); only MR_BC_LINE_TIED is implemented */
+    mr_bc bc[3];            /* per logical axis (both faces) */
     double gamma;           /* > 0; Eq. 1.5, the paper uses 1 (:55) */
     mr_dtype dtype;         /* storage and arithmetic type of the state; reductions always accumulate in fp64 */
     void* workspace;        /* device pointer, >= mr_workspace_bytes(), 256-byte aligned, caller-owned */
@@ -83,7 +87,8 @@ typedef struct {
  * reduction partials; about 4 fields = 12*nx*ny*nz elements.  Pure host arithmetic, needs no GPU. */
 size_t mr_workspace_bytes(const mr_grid* grid, mr_dtype dtype);
 
-/* Create a context on the current CUDA device; the state is initialised to x = X.
+/* Create a context on the current CUDA device; the state is initialised to x = X, so a run that starts on
+ * the reference grid needs no mr_set_x.
  * Returns MR_ERR_INVALID_ARG for bad sizes/options (checked before any CUDA call), MR_ERR_WORKSPACE,
  * MR_ERR_CUDA (e.g. no sm_100 device).  On failure *out is NULL. */
 mr_status mr_create(const mr_grid* grid, const mr_domain* domain, const mr_boundary* boundary, mr_ctx** out);
@@ -102,6 +107,12 @@ mr_status mr_set_B0_host(mr_ctx* ctx, const void* B0_host);
 mr_status mr_set_x(mr_ctx* ctx, const void* x_dev);
 mr_status mr_set_x_host(mr_ctx* ctx, const void* x_host);
 
+/* The same through the DISPLACEMENT xi = x - X (dense, context dtype): on an fp32 context positions lose eps*|X| per
+ * node at the ABI, 300 times the rounding of xi itself (reading Q15), so fp32 callers exchange xi.  Nodes on
+ * line-tied faces must have |xi| <= 1e-6*h.  mr_get_xi is asynchronous. */
+mr_status mr_set_xi(mr_ctx* ctx, const void* xi_dev);
+mr_status mr_get_xi(mr_ctx* ctx, void* xi_dev);
+
 /* Take n >= 0 explicit steps x <- x + dt * gamma * J x B on interior nodes, boundary nodes fixed (Eq. 1.2,
  * :17; :147), all velocities from the old x.  dt > 0.  Synchronises the stream at the end and returns
  * MR_ERR_NUMERIC if any node had det <= 0 or a non-finite value during these steps, MR_ERR_STATE without B0. */
@@ -117,6 +128,49 @@ mr_status mr_diagnostics(mr_ctx* ctx, mr_operator op, mr_diag* out);
 mr_status mr_get_fields(mr_ctx* ctx, mr_operator op, void* x_dev, void* B_dev, void* J_dev);
 mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_host, void* B_host, void* J_host);
 
+/* The velocity u = gamma J x B (Eq. 1.5, :40) of the current state, dense, context dtype, 0 on line-tied boundary
+ * nodes: the right-hand side of dx/dt = u that mr_step and mr_step_adaptive integrate.  Asynchronous. */
+mr_status mr_rhs(mr_ctx* ctx, mr_operator op, void* u_dev);
+
+/* ---- section 2.4 (:131-143): adaptive Cash-Karp RK5(4) with the step control of Eq. 2.11 -------------------------
+ * Needs a second caller-owned device buffer for the six stage velocities and the stage state (7 fields), bound once. */
+size_t mr_adaptive_workspace_bytes(const mr_grid* grid, mr_dtype dtype);
+mr_status mr_bind_adaptive_workspace(mr_ctx* ctx, void* workspace_dev, size_t bytes);
+
+typedef struct {
+    int64_t accepted, rejected; /* trial steps of this call */
+    int64_t rhs_evals;          /* 6 per trial */
+    double time;                /* reached (== t_end unless max_trials ran out or the run failed) */
+    double dt_next;             /* step length handed on (also written to *dt) */
+    double last_lambda;         /* Lambda = max |x5 - x4| of the last trial */
+} mr_adapt_stats;
+
+/* Integrate from the context's time to t_end.  Each trial step evaluates u six times (the RHS instantiation of the
+ * step kernels), forms the fifth-order solution and Lambda = max over nodes and components of |x5 - x4| on the device
+ * and brings ONE scalar back; the host rejects the trial if Lambda > lambda0 and retries with dt' = dt |lambda0/Lambda|^0.2
+ * (Eq. 2.11), accepts it otherwise and enlarges dt by the same formula if Lambda < lambda0/2 (growth capped at 5x).
+ * The last step is clipped to end at t_end.  *dt: first trial step in, step handed on out.  trace_host (may be NULL):
+ * trace_cap rows {t, dt tried, Lambda, accepted} of the trials.  Returns MR_ERR_STATE without B0 or without the
+ * adaptive workspace, MR_ERR_NUMERIC if a stage met det <= 0 (the state is then the last accepted one),
+ * MR_ERR_INVALID_ARG if max_trials ran out before t_end. */
+mr_status mr_step_adaptive(mr_ctx* ctx, double t_end, double lambda0, double* dt, mr_operator op, int64_t max_trials,
+                           mr_adapt_stats* stats, double* trace_host, int64_t trace_cap);
+
+/* ---- section 3.2 diagnostics beyond E_M and xi ------------------------------------------------------------------
+ * Convexity (Eqs. 3.10-3.11, :231-243): kappa = +1 where every trihedron of the node (three nearest neighbours, one per
+ * axis, all that exist) has sgn det = di dj dk, else -1, into kappa_dev (dense int32[nz][ny][nx], may be NULL); the
+ * number of nodes with kappa = -1 into *n_concave (the early warning of :333). */
+mr_status mr_convexity(mr_ctx* ctx, int32_t* kappa_dev, int64_t* n_concave);
+
+/* alpha* = J.B/B^2 (Eq. 3.5, :206) at the inner nodes of the grid line (ic, jc, .) -- s_alpha of Eq. 3.6 when the line
+ * is the z axis -- into alpha_host[nz] (may be NULL; 0 at line-tied end nodes), and
+ * eps* = max over pairs of a_r (alpha*_i - alpha*_j)/|X_i - X_j| (Eq. 3.7, :214) into *eps_star. */
+mr_status mr_eps_star(mr_ctx* ctx, mr_operator op, int32_t ic, int32_t jc, double a_r, double* alpha_host, double* eps_star);
+
+/* sigma_x and sigma_B (Eqs. 3.9, 3.8, :221-229): root mean square over ALL nodes of |x - x_ref| and |B - B_ref|;
+ * the references are dense device arrays in the context dtype (for the IsoHelix field Eqs. 3.3 and 3.2). */
+mr_status mr_sigma(mr_ctx* ctx, const void* x_ref_dev, const void* B_ref_dev, double* sigma_x, double* sigma_B);
+
 /* Message for the last error on this context ("" if none); ctx == NULL gives the last mr_create failure.
  * The pointer stays valid until the next failing call on the same context (or mr_destroy). */
 const char* mr_last_error(const mr_ctx* ctx);
@@ -127,7 +181,7 @@ int64_t mr_launch_count(const mr_ctx* ctx);
 const char* mr_step_variant(const mr_ctx* ctx);
 
 /* Choose the step kernel.  "auto" (default): the streaming TMA kernels (mimetic: csrc/mr_sym.cuh, direct:
- * csrc/mr_direct.cuh).  "generic": the global-memory kernels of csrc/mr_generic.cuh for both operators (one thread per
+ * csrc/mr_direct.cuh) when every axis is line-tied.  "generic": the global-memory kernels of csrc/mr_generic.cuh for both operators (one thread per
  * node, every stencil value straight from global memory): the A/B reference of the tests.  Both agree to rounding. */
 mr_status mr_set_variant(mr_ctx* ctx, const char* name);
 

@@ -1,4 +1,5 @@
-// mr_api.cu -- the C-ABI of include/mr.h: argument validation, workspace carving, kernel launches.
+// mr_api.cu -- the C-ABI of include/mr.h: argument validation, workspace carving, kernel launches, and the host side of
+// the adaptive integrator (accept / reject, Eq. 2.11).
 #include "../../include/mr.h"
 
 #include <cmath>
@@ -12,6 +13,7 @@
 #include "mr_stream_common.cuh"
 #include "mr_direct.cuh"
 #include "mr_sym.cuh"
+#include "mr_next.cuh"
 
 using namespace mr;
 
@@ -28,6 +30,7 @@ struct Layout {
     size_t field_bytes;   // one padded 3-component field
     size_t stage_bytes;   // one dense 3-component field
     size_t off_xi[2], off_b, off_stage, off_partials, off_diag, off_flag, total;
+    size_t adaptive_total;   // the second workspace: 7 padded fields
 };
 
 bool make_layout(const mr_grid* g, mr_dtype dt, Layout* L)
@@ -46,10 +49,11 @@ bool make_layout(const mr_grid* g, mr_dtype dt, Layout* L)
     L->off_xi[1] = o; o += L->field_bytes;
     L->off_b = o; o += L->field_bytes;
     L->off_stage = o; o += L->stage_bytes;
-    L->off_partials = o; o += align_up(sizeof(DiagPartial) * kMaxPartialBlocks, kAlign);
+    L->off_partials = o; o += align_up(sizeof(DiagPartial) * (2 * kMaxPartialBlocks), kAlign);
     L->off_diag = o; o += kAlign;
     L->off_flag = o; o += kAlign;
     L->total = o;
+    L->adaptive_total = 7 * L->field_bytes;
     return true;
 }
 
@@ -63,8 +67,11 @@ struct mr_ctx {
     mr_dtype dtype;
     double gamma;
     double h[3];
+    int per[3];
+    bool any_periodic;
     Layout L;
     char* ws;
+    char* aws;          // adaptive workspace (k_1 .. k_6, stage state) or null
     cudaStream_t stream;
     int cur;            // which xi buffer holds the current state
     bool have_B0;
@@ -75,8 +82,9 @@ struct mr_ctx {
     int sm_count;
     int force_variant;  // 0 auto (streaming kernels), 1 generic (global-memory kernels, the A/B reference)
     const char* variant;
-    StreamPlan plan6;   // the streaming kernel of the direct-derivative operator (mr_direct.cuh)
-    StreamPlan plan7;   // the symmetric split-phase streaming kernel of the mimetic operator (mr_sym.cuh)
+    bool plans_built;
+    StreamPlan plan_dir;   // the streaming kernel of the direct-derivative operator (mr_direct.cuh)
+    StreamPlan plan_mim;   // the streaming kernel of the mimetic operator (mr_sym.cuh)
     std::string err;
 
     void* xi(int w) const { return ws + L.off_xi[w]; }
@@ -85,6 +93,7 @@ struct mr_ctx {
     DiagPartial* partials() const { return reinterpret_cast<DiagPartial*>(ws + L.off_partials); }
     DiagPartial* diag_out() const { return reinterpret_cast<DiagPartial*>(ws + L.off_diag); }
     int* flag() const { return reinterpret_cast<int*>(ws + L.off_flag); }
+    void* kbuf(int s) const { return aws + (size_t)s * L.field_bytes; }      // s = 0..5: k_1..k_6, 6: the stage state
     size_t esize() const { return dtype == MR_F64 ? 8 : 4; }
     size_t dense_bytes() const { return (size_t)3 * grid.nx * grid.ny * grid.nz * esize(); }
 };
@@ -114,7 +123,7 @@ GridP<T> grid_params(const mr_ctx* c)
     GridP<T> g;
     g.nx = c->grid.nx; g.ny = c->grid.ny; g.nz = c->grid.nz;
     g.pitch = c->L.pitch; g.plane = c->L.plane; g.comp = c->L.comp;
-    for (int a = 0; a < 3; ++a) g.twoh[a] = (T)(2.0 * c->h[a]);
+    for (int a = 0; a < 3; ++a) { g.twoh[a] = (T)(2.0 * c->h[a]); g.per[a] = c->per[a]; }
     return g;
 }
 
@@ -138,6 +147,41 @@ mr_status read_flag(mr_ctx* c, int* out)
     return MR_OK;
 }
 
+// the TMA descriptors and launch geometry of the streaming kernels, on first use
+void ensure_plans(mr_ctx* c)
+{
+    if (c->plans_built) return;
+    c->plans_built = true;
+    StreamGeom sg;
+    sg.nx = c->grid.nx; sg.ny = c->grid.ny; sg.nz = c->grid.nz;
+    sg.pitch = c->L.pitch; sg.plane = c->L.plane; sg.comp = c->L.comp;
+    for (int a = 0; a < 3; ++a) sg.twoh[a] = 2.0 * c->h[a];
+    std::string why;
+    if (c->any_periodic) {       // the TMA boxes rely on zero fill outside the grid: line-tied faces only
+        c->plan_dir.usable = c->plan_mim.usable = false;
+        return;
+    }
+    if (!build_direct_plan(&c->plan_dir, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+        c->plan_dir.usable = false;
+        c->plan_dir.why = why;
+    }
+    if (!build_sym_plan(&c->plan_mim, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+        c->plan_mim.usable = false;
+        c->plan_mim.why = why;
+    }
+    if (c->aws) {
+        if (c->plan_mim.usable && !sym_bind_stage(&c->plan_mim, c->kbuf(6))) c->plan_mim.usable = false;
+        if (c->plan_dir.usable && !direct_bind_stage(&c->plan_dir, c->kbuf(6))) c->plan_dir.usable = false;
+    }
+}
+
+bool streaming(mr_ctx* c, mr_operator op)
+{
+    ensure_plans(c);
+    if (c->force_variant != 0) return false;
+    return op == MR_OP_MIMETIC ? c->plan_mim.usable : c->plan_dir.usable;
+}
+
 template <typename T>
 mr_status do_set_B0(mr_ctx* c, const void* B0_dev)
 {
@@ -152,15 +196,19 @@ mr_status do_set_B0(mr_ctx* c, const void* B0_dev)
     return MR_OK;
 }
 
+// x (as_xi = false) or xi (as_xi = true), dense -> the other state buffer; adopted if the line-tied faces are on X
 template <typename T>
-mr_status do_set_x(mr_ctx* c, const void* x_dev)
+mr_status do_set_x(mr_ctx* c, const void* src, bool as_xi)
 {
     dim3 grid, block;
     node_launch_dims(c, grid, block);
     const int other = 1 - c->cur;
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
-    k_import_x<T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(x_dev), static_cast<T*>(c->xi(other)),
-                                                 grid_params<T>(c), domain_params(c), c->flag());
+    if (as_xi)
+        k_import_xi<T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(src), static_cast<T*>(c->xi(other)), grid_params<T>(c), c->flag());
+    else
+        k_import_x<T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(src), static_cast<T*>(c->xi(other)), grid_params<T>(c),
+                                                     domain_params(c), c->flag());
     c->launches++;
     MR_CUDA(c, cudaGetLastError());
     int f = 0;
@@ -183,29 +231,43 @@ mr_status do_fields(mr_ctx* c, mr_operator op, void* x_out, void* B_out, void* J
     const T* xi = static_cast<const T*>(c->xi(c->cur));
     const T* b = static_cast<const T*>(c->b());
     if (op == MR_OP_MIMETIC)
-        k_fields<T, 0><<<grid, block, 0, c->stream>>>(xi, b, grid_params<T>(c), domain_params(c), static_cast<T*>(x_out),
+        k_fields<T, 0><<<grid, block, 0, c->stream>>>(xi, b, grid_params<double>(c), domain_params(c), static_cast<T*>(x_out),
                                                       static_cast<T*>(B_out), static_cast<T*>(J_out), c->flag());
     else
-        k_fields<T, 1><<<grid, block, 0, c->stream>>>(xi, b, grid_params<T>(c), domain_params(c), static_cast<T*>(x_out),
+        k_fields<T, 1><<<grid, block, 0, c->stream>>>(xi, b, grid_params<double>(c), domain_params(c), static_cast<T*>(x_out),
                                                       static_cast<T*>(B_out), static_cast<T*>(J_out), c->flag());
     c->launches++;
     MR_CUDA(c, cudaGetLastError());
     return MR_OK;
 }
 
+// One pass of the hot path over the state in buffer `in` (0, 1: the state buffers, 2: the adaptive stage buffer):
+// rhs = false: out = xi + dtg J x B (a step), rhs = true: out = dtg J x B (the velocity for dtg = gamma).
 template <typename T>
-mr_status launch_generic_step(mr_ctx* c, double dt, mr_operator op)
+mr_status launch_pass(mr_ctx* c, mr_operator op, int in, void* out, double dtg_d, bool rhs)
 {
-    dim3 grid, block;
-    node_launch_dims(c, grid, block);
-    const T* in = static_cast<const T*>(c->xi(c->cur));
-    T* out = static_cast<T*>(c->xi(1 - c->cur));
-    const T* b = static_cast<const T*>(c->b());
-    const T dtg = (T)(dt * c->gamma);
-    if (op == MR_OP_MIMETIC)
-        k_step_generic<T, 0><<<grid, block, 0, c->stream>>>(in, out, b, grid_params<T>(c), dtg, c->flag());
-    else
-        k_step_generic<T, 1><<<grid, block, 0, c->stream>>>(in, out, b, grid_params<T>(c), dtg, c->flag());
+    const T dtg = (T)dtg_d;
+    if (streaming(c, op)) {
+        cudaError_t e = op == MR_OP_MIMETIC ? launch_sym_step<T>(c->plan_mim, in, dtg, c->flag(), c->stream, rhs, out)
+                                            : launch_direct_step<T>(c->plan_dir, in, dtg, c->flag(), c->stream, rhs, out);
+        if (e != cudaSuccess) return cuda_fail(c, "streaming step launch", e);
+        c->variant = op == MR_OP_MIMETIC ? c->plan_mim.name : c->plan_dir.name;
+    } else {
+        dim3 grid, block;
+        node_launch_dims(c, grid, block);
+        const T* src = static_cast<const T*>(in == 2 ? c->kbuf(6) : c->xi(in));
+        const T* b = static_cast<const T*>(c->b());
+        T* o = static_cast<T*>(out);
+        const GridP<T> g = grid_params<T>(c);
+        if (op == MR_OP_MIMETIC) {
+            if (rhs) k_step_generic<T, 0, true><<<grid, block, 0, c->stream>>>(src, o, b, g, dtg, c->flag());
+            else k_step_generic<T, 0, false><<<grid, block, 0, c->stream>>>(src, o, b, g, dtg, c->flag());
+        } else {
+            if (rhs) k_step_generic<T, 1, true><<<grid, block, 0, c->stream>>>(src, o, b, g, dtg, c->flag());
+            else k_step_generic<T, 1, false><<<grid, block, 0, c->stream>>>(src, o, b, g, dtg, c->flag());
+        }
+        c->variant = op == MR_OP_MIMETIC ? "generic_mimetic" : "generic_direct";
+    }
     c->launches++;
     return MR_OK;
 }
@@ -213,21 +275,10 @@ mr_status launch_generic_step(mr_ctx* c, double dt, mr_operator op)
 template <typename T>
 mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
 {
-    const bool mim = op == MR_OP_MIMETIC;
-    const bool use_sym = mim && c->force_variant == 0 && c->plan7.usable;
-    const bool use_dstream = !mim && c->force_variant == 0 && c->plan6.usable;
-    c->variant = use_dstream ? c->plan6.name : use_sym ? c->plan7.name : (mim ? "generic_mimetic" : "generic_direct");
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     for (int64_t s = 0; s < n; ++s) {
-        if (use_dstream || use_sym) {
-            const T dtg = (T)(dt * c->gamma);
-            cudaError_t e = use_dstream ? launch_direct_step<T>(c->plan6, c->cur, dtg, c->flag(), c->stream)
-                                        : launch_sym_step<T>(c->plan7, c->cur, dtg, c->flag(), c->stream);
-            if (e != cudaSuccess) return cuda_fail(c, "streaming step launch", e);
-            c->launches++;
-        } else {
-            launch_generic_step<T>(c, dt, op);
-        }
+        mr_status st = launch_pass<T>(c, op, c->cur, c->xi(1 - c->cur), dt * c->gamma, false);
+        if (st != MR_OK) return st;
         c->cur = 1 - c->cur;
     }
     MR_CUDA(c, cudaGetLastError());
@@ -254,18 +305,30 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     const T* b = static_cast<const T*>(c->b());
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     const int threads = c->grid.nx >= 256 ? 256 : (c->grid.nx >= 128 ? 128 : (c->grid.nx >= 64 ? 64 : 32));
-    const bool fused = op == MR_OP_MIMETIC && c->plan7.usable && c->force_variant == 0 &&
-                       c->plan7.tiles_x * c->plan7.tiles_y * c->plan7.nchunks <= kMaxPartialBlocks;
-    if (fused) {
-        // the streaming pass of the step kernel with the update replaced by the reduction (mr_sym.cuh, DIAG)
-        cudaError_t e = launch_sym_diag<T>(c->plan7, c->cur, c->partials(), &blocks, c->flag(), c->stream);
+    const bool stream_ok = streaming(c, op);
+    const StreamPlan& pl = op == MR_OP_MIMETIC ? c->plan_mim : c->plan_dir;
+    const bool fused = stream_ok && pl.tiles_x * pl.tiles_y * pl.nchunks <= kMaxPartialBlocks;
+    int total = blocks;
+    if (fused && op == MR_OP_MIMETIC) {
+        // the streaming pass of the step kernel with the update replaced by the reduction (mr_sym.cuh, MODE_DIAG)
+        cudaError_t e = launch_sym_diag<T>(c->plan_mim, c->cur, c->partials(), &total, c->flag(), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, "streaming diagnostics launch", e);
-    } else if (op == MR_OP_MIMETIC)
-        k_diag<T, 0><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());
-    else
-        k_diag<T, 1><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());
-    k_diag_final<<<1, 256, 0, c->stream>>>(c->partials(), blocks, c->diag_out());
-    c->launches += 2;
+        c->launches++;
+    } else if (fused) {
+        // direct operator: the inner nodes by the streaming pass, the nodes on the faces by a pass of their own
+        int inner_blocks = 0;
+        cudaError_t e = launch_direct_diag<T>(c->plan_dir, c->cur, c->partials(), &inner_blocks, c->flag(), c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, "streaming diagnostics launch", e);
+        k_diag_faces<T><<<blocks, 128, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials() + inner_blocks, c->flag());
+        total = inner_blocks + blocks;
+        c->launches += 2;
+    } else {
+        if (op == MR_OP_MIMETIC) k_diag<T, 0><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());
+        else k_diag<T, 1><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());
+        c->launches++;
+    }
+    k_diag_final<<<1, 256, 0, c->stream>>>(c->partials(), total, c->diag_out());
+    c->launches++;
     MR_CUDA(c, cudaGetLastError());
     DiagPartial r;
     MR_CUDA(c, cudaMemcpyAsync(&r, c->diag_out(), sizeof(r), cudaMemcpyDeviceToHost, c->stream));
@@ -283,6 +346,142 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     return MR_OK;
 }
 
+// ---- section 2.4: one Cash-Karp trial step of length h from the state buffer `cur`; the fifth-order solution goes
+// to the other state buffer, Lambda = max |x5 - x4| comes back (the one device -> host scalar of the step)
+template <typename T>
+mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* numeric)
+{
+    static const CashKarp ck = cash_karp();
+    const long long n2 = 3 * c->L.comp / 2;             // element pairs of a padded field (pitch is a multiple of 16)
+    const int blocks = c->sm_count * 8 < kMaxPartialBlocks ? c->sm_count * 8 : kMaxPartialBlocks;
+    const T* x = static_cast<const T*>(c->xi(c->cur));
+    T* xs = static_cast<T*>(c->kbuf(6));
+    MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
+    for (int s = 0; s < 6; ++s) {
+        if (s > 0) {
+            StageArgs a;
+            a.n = s;
+            for (int r = 0; r < 6; ++r) { a.k[r] = c->kbuf(r < s ? r : 0); a.c[r] = r < s ? h * ck.a[s][r] : 0.0; }
+            k_rk_stage<T><<<blocks, 256, 0, c->stream>>>(x, xs, a, n2);
+            c->launches++;
+        }
+        mr_status st = launch_pass<T>(c, op, s == 0 ? c->cur : 2, c->kbuf(s), c->gamma, true);
+        if (st != MR_OK) return st;
+    }
+    StageArgs b5, db;
+    b5.n = db.n = 6;
+    for (int r = 0; r < 6; ++r) { b5.k[r] = db.k[r] = c->kbuf(r); b5.c[r] = h * ck.b5[r]; db.c[r] = h * ck.db[r]; }
+    double* partial = reinterpret_cast<double*>(c->partials());
+    k_rk_final<T><<<blocks, 256, 0, c->stream>>>(x, static_cast<T*>(c->xi(1 - c->cur)), b5, db, n2, partial);
+    k_max_final<<<1, 256, 0, c->stream>>>(partial, blocks, reinterpret_cast<double*>(c->diag_out()));
+    c->launches += 2;
+    MR_CUDA(c, cudaGetLastError());
+    MR_CUDA(c, cudaMemcpyAsync(lambda, c->diag_out(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    return read_flag(c, numeric);
+}
+
+// Eq. 2.11 and the accept / reject rule of PAPER.md:139-143 (reading Q22)
+bool step_control(double dt, double lambda, double lambda0, double* dt_next)
+{
+    if (lambda > lambda0 || lambda != lambda) {
+        *dt_next = lambda != lambda ? 0.5 * dt : dt * std::pow(std::fabs(lambda0 / lambda), 0.2);
+        return false;
+    }
+    if (lambda < 0.5 * lambda0) {
+        const double f = lambda > 0.0 ? std::pow(std::fabs(lambda0 / lambda), 0.2) : 5.0;
+        *dt_next = dt * (f > 5.0 ? 5.0 : f);
+    } else {
+        *dt_next = dt;
+    }
+    return true;
+}
+
+template <typename T>
+mr_status do_adaptive(mr_ctx* c, double t_end, double lambda0, double* dt, mr_operator op, int64_t max_trials, mr_adapt_stats* stats,
+                      double* trace, int64_t trace_cap)
+{
+    mr_adapt_stats s = { 0, 0, 0, c->time, *dt, 0.0 };
+    int64_t trials = 0;
+    mr_status rc = MR_OK;
+    while (c->time < t_end) {
+        if (trials >= max_trials) { rc = fail(c, MR_ERR_INVALID_ARG, "mr_step_adaptive: max_trials exhausted before t_end"); break; }
+        const double rest = t_end - c->time;
+        const bool clipped = *dt >= rest;
+        const double h = clipped ? rest : *dt;
+        double lam = 0.0, dt_next = 0.0;
+        int numeric = 0;
+        rc = rk_trial<T>(c, op, h, &lam, &numeric);
+        if (rc != MR_OK) break;
+        s.rhs_evals += 6;
+        if (numeric & FLAG_NUMERIC) lam = NAN;           // a stage folded the grid: the trial counts as failed
+        s.last_lambda = lam;
+        const bool ok = step_control(h, lam, lambda0, &dt_next);
+        if (trace && trials < trace_cap) {
+            trace[4 * trials + 0] = c->time; trace[4 * trials + 1] = h; trace[4 * trials + 2] = lam; trace[4 * trials + 3] = ok ? 1.0 : 0.0;
+        }
+        ++trials;
+        if (ok) {
+            c->cur = 1 - c->cur;
+            c->time = clipped ? t_end : c->time + h;
+            c->steps++;
+            s.accepted++;
+            if (!clipped || dt_next < *dt) *dt = dt_next;     // a clipped last step does not change the dt handed on
+        } else {
+            s.rejected++;
+            *dt = dt_next;
+            if (!(dt_next > 1e-300)) { rc = fail(c, MR_ERR_NUMERIC, "mr_step_adaptive: the step length collapsed (cf. PAPER.md:333)"); break; }
+        }
+    }
+    s.time = c->time;
+    s.dt_next = *dt;
+    if (stats) *stats = s;
+    return rc;
+}
+
+template <typename T>
+mr_status do_eps_star(mr_ctx* c, mr_operator op, int ic, int jc, double a_r, double* alpha_host, double* eps)
+{
+    double* alpha = reinterpret_cast<double*>(c->partials());          // nz <= 4096 doubles fit the partials area
+    const T* xi = static_cast<const T*>(c->xi(c->cur));
+    const T* b = static_cast<const T*>(c->b());
+    MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
+    const int nz = c->grid.nz;
+    if (op == MR_OP_MIMETIC) k_alpha_line<T, 0><<<(nz + 63) / 64, 64, 0, c->stream>>>(xi, b, grid_params<T>(c), ic, jc, alpha, c->flag());
+    else k_alpha_line<T, 1><<<(nz + 63) / 64, 64, 0, c->stream>>>(xi, b, grid_params<T>(c), ic, jc, alpha, c->flag());
+    const int k_lo = c->per[2] ? 0 : 1, k_hi = c->per[2] ? nz - 1 : nz - 2;
+    k_eps_star<<<1, 256, 0, c->stream>>>(alpha, k_lo, k_hi, a_r, c->h[2], reinterpret_cast<double*>(c->diag_out()));
+    c->launches += 2;
+    MR_CUDA(c, cudaGetLastError());
+    if (alpha_host) MR_CUDA(c, cudaMemcpyAsync(alpha_host, alpha, sizeof(double) * nz, cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaMemcpyAsync(eps, c->diag_out(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    int f = 0;
+    mr_status st = read_flag(c, &f);
+    if (st != MR_OK) return st;
+    if (f & FLAG_NUMERIC) return fail(c, MR_ERR_NUMERIC, "mr_eps_star: det(dx/dX) <= 0 on the line");
+    return MR_OK;
+}
+
+template <typename T>
+mr_status do_sigma(mr_ctx* c, const void* x_ref, const void* B_ref, double* sx, double* sb)
+{
+    const long long rows = (long long)c->grid.ny * c->grid.nz;
+    int blocks = c->sm_count * 8 < kMaxPartialBlocks ? c->sm_count * 8 : kMaxPartialBlocks;
+    if (blocks > rows) blocks = (int)rows;
+    SumPair* partials = reinterpret_cast<SumPair*>(c->partials());
+    k_sigma<T><<<blocks, 256, 0, c->stream>>>(static_cast<const T*>(c->xi(c->cur)), static_cast<const T*>(c->b()), grid_params<T>(c),
+                                              domain_params(c), static_cast<const T*>(x_ref), static_cast<const T*>(B_ref), partials);
+    k_sum_final<<<1, 32, 0, c->stream>>>(partials, blocks, reinterpret_cast<SumPair*>(c->diag_out()));
+    c->launches += 2;
+    MR_CUDA(c, cudaGetLastError());
+    SumPair r;
+    MR_CUDA(c, cudaMemcpyAsync(&r, c->diag_out(), sizeof(r), cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    const double N = (double)c->grid.nx * c->grid.ny * c->grid.nz;
+    *sx = std::sqrt(r.a / N);
+    *sb = std::sqrt(r.b / N);
+    return MR_OK;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------- C ABI
@@ -291,6 +490,12 @@ extern "C" size_t mr_workspace_bytes(const mr_grid* grid, mr_dtype dtype)
 {
     Layout L;
     return make_layout(grid, dtype, &L) ? L.total : 0;
+}
+
+extern "C" size_t mr_adaptive_workspace_bytes(const mr_grid* grid, mr_dtype dtype)
+{
+    Layout L;
+    return make_layout(grid, dtype, &L) ? L.adaptive_total : 0;
 }
 
 extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, const mr_boundary* boundary, mr_ctx** out)
@@ -303,9 +508,8 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     for (int a = 0; a < 3; ++a) {
         if (!std::isfinite(domain->lo[a]) || !std::isfinite(domain->hi[a]) || !(domain->hi[a] > domain->lo[a]))
             return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: domain needs finite hi > lo on every axis");
-        if (boundary->bc[a] == MR_BC_PERIODIC)
-            return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: periodic boundaries (Eqs. 2.12-2.14) are not implemented");
-        if (boundary->bc[a] != MR_BC_LINE_TIED) return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: unknown boundary type");
+        if (boundary->bc[a] != MR_BC_LINE_TIED && boundary->bc[a] != MR_BC_PERIODIC)
+            return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: unknown boundary type");
     }
     if (!(boundary->gamma > 0.0) || !std::isfinite(boundary->gamma))
         return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: gamma must be finite and > 0");
@@ -328,9 +532,15 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     c->dtype = boundary->dtype;
     c->gamma = boundary->gamma;
     const int n[3] = { grid->nx, grid->ny, grid->nz };
-    for (int a = 0; a < 3; ++a) c->h[a] = (domain->hi[a] - domain->lo[a]) / (double)(n[a] - 1);
+    c->any_periodic = false;
+    for (int a = 0; a < 3; ++a) {
+        c->h[a] = (domain->hi[a] - domain->lo[a]) / (double)(n[a] - 1);
+        c->per[a] = boundary->bc[a] == MR_BC_PERIODIC ? 1 : 0;
+        c->any_periodic = c->any_periodic || c->per[a];
+    }
     c->L = L;
     c->ws = static_cast<char*>(boundary->workspace);
+    c->aws = nullptr;
     c->stream = static_cast<cudaStream_t>(boundary->stream);
     c->cur = 0;
     c->have_B0 = false;
@@ -341,24 +551,11 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     c->sm_count = prop.multiProcessorCount;
     c->force_variant = 0;
     c->variant = "";
+    c->plans_built = false;
 
     cudaError_t e = cudaMemsetAsync(c->ws, 0, L.off_stage, c->stream);   // xi = 0 (x = X), b = 0, incl. padding
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.off_partials, 0, L.total - L.off_partials, c->stream);
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, "mr_create: cudaMemsetAsync", e); }
-
-    StreamGeom sg;
-    sg.nx = grid->nx; sg.ny = grid->ny; sg.nz = grid->nz;
-    sg.pitch = L.pitch; sg.plane = L.plane; sg.comp = L.comp;
-    for (int a = 0; a < 3; ++a) sg.twoh[a] = 2.0 * c->h[a];
-    std::string why;
-    if (!build_direct_plan(&c->plan6, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan6.usable = false;
-        c->plan6.why = why;
-    }
-    if (!build_sym_plan(&c->plan7, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
-        c->plan7.usable = false;
-        c->plan7.why = why;
-    }
     *out = c;
     return MR_OK;
 }
@@ -391,7 +588,7 @@ extern "C" mr_status mr_set_x(mr_ctx* ctx, const void* x_dev)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
     if (!x_dev) return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_x: null pointer");
-    return ctx->dtype == MR_F64 ? do_set_x<double>(ctx, x_dev) : do_set_x<float>(ctx, x_dev);
+    return ctx->dtype == MR_F64 ? do_set_x<double>(ctx, x_dev, false) : do_set_x<float>(ctx, x_dev, false);
 }
 
 extern "C" mr_status mr_set_x_host(mr_ctx* ctx, const void* x_host)
@@ -400,6 +597,28 @@ extern "C" mr_status mr_set_x_host(mr_ctx* ctx, const void* x_host)
     if (!x_host) return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_x_host: null pointer");
     MR_CUDA(ctx, cudaMemcpyAsync(ctx->stage(), x_host, ctx->dense_bytes(), cudaMemcpyHostToDevice, ctx->stream));
     return mr_set_x(ctx, ctx->stage());
+}
+
+extern "C" mr_status mr_set_xi(mr_ctx* ctx, const void* xi_dev)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!xi_dev) return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_xi: null pointer");
+    return ctx->dtype == MR_F64 ? do_set_x<double>(ctx, xi_dev, true) : do_set_x<float>(ctx, xi_dev, true);
+}
+
+extern "C" mr_status mr_get_xi(mr_ctx* ctx, void* xi_dev)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!xi_dev) return fail(ctx, MR_ERR_INVALID_ARG, "mr_get_xi: null pointer");
+    dim3 grid, block;
+    node_launch_dims(ctx, grid, block);
+    if (ctx->dtype == MR_F64)
+        k_export_padded<double><<<grid, block, 0, ctx->stream>>>(static_cast<const double*>(ctx->xi(ctx->cur)), static_cast<double*>(xi_dev), grid_params<double>(ctx));
+    else
+        k_export_padded<float><<<grid, block, 0, ctx->stream>>>(static_cast<const float*>(ctx->xi(ctx->cur)), static_cast<float*>(xi_dev), grid_params<float>(ctx));
+    ctx->launches++;
+    MR_CUDA(ctx, cudaGetLastError());
+    return MR_OK;
 }
 
 extern "C" mr_status mr_step(mr_ctx* ctx, int64_t n, double dt, mr_operator op)
@@ -412,6 +631,58 @@ extern "C" mr_status mr_step(mr_ctx* ctx, int64_t n, double dt, mr_operator op)
     return ctx->dtype == MR_F64 ? do_step<double>(ctx, n, dt, op) : do_step<float>(ctx, n, dt, op);
 }
 
+extern "C" mr_status mr_rhs(mr_ctx* ctx, mr_operator op, void* u_dev)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!u_dev) return fail(ctx, MR_ERR_INVALID_ARG, "mr_rhs: null pointer");
+    if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_rhs: unknown operator");
+    if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_rhs: B0 has not been set");
+    // the velocity in the padded layout into the spare state buffer, then dense into the caller's array
+    void* tmp = ctx->xi(1 - ctx->cur);
+    mr_status st = ctx->dtype == MR_F64 ? launch_pass<double>(ctx, op, ctx->cur, tmp, ctx->gamma, true)
+                                        : launch_pass<float>(ctx, op, ctx->cur, tmp, ctx->gamma, true);
+    if (st != MR_OK) return st;
+    dim3 grid, block;
+    node_launch_dims(ctx, grid, block);
+    if (ctx->dtype == MR_F64)
+        k_export_padded<double><<<grid, block, 0, ctx->stream>>>(static_cast<const double*>(tmp), static_cast<double*>(u_dev), grid_params<double>(ctx));
+    else
+        k_export_padded<float><<<grid, block, 0, ctx->stream>>>(static_cast<const float*>(tmp), static_cast<float*>(u_dev), grid_params<float>(ctx));
+    ctx->launches++;
+    MR_CUDA(ctx, cudaGetLastError());
+    return MR_OK;
+}
+
+extern "C" mr_status mr_bind_adaptive_workspace(mr_ctx* ctx, void* workspace_dev, size_t bytes)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) % kAlign) != 0)
+        return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_adaptive_workspace: workspace is null or not 256-byte aligned");
+    if (bytes < ctx->L.adaptive_total)
+        return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_adaptive_workspace: smaller than mr_adaptive_workspace_bytes()");
+    ctx->aws = static_cast<char*>(workspace_dev);
+    MR_CUDA(ctx, cudaMemsetAsync(ctx->aws, 0, ctx->L.adaptive_total, ctx->stream));       // the padding must stay finite
+    if (ctx->plans_built) {
+        if (ctx->plan_mim.usable && !sym_bind_stage(&ctx->plan_mim, ctx->kbuf(6))) ctx->plan_mim.usable = false;
+        if (ctx->plan_dir.usable && !direct_bind_stage(&ctx->plan_dir, ctx->kbuf(6))) ctx->plan_dir.usable = false;
+    }
+    return MR_OK;
+}
+
+extern "C" mr_status mr_step_adaptive(mr_ctx* ctx, double t_end, double lambda0, double* dt, mr_operator op, int64_t max_trials,
+                                      mr_adapt_stats* stats, double* trace_host, int64_t trace_cap)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!dt || !(*dt > 0.0) || !std::isfinite(*dt) || !(lambda0 > 0.0) || !std::isfinite(t_end) || max_trials < 0)
+        return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_adaptive: need finite t_end, lambda0 > 0, *dt > 0, max_trials >= 0");
+    if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_adaptive: unknown operator");
+    if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_step_adaptive: B0 has not been set");
+    if (!ctx->aws) return fail(ctx, MR_ERR_STATE, "mr_step_adaptive: no adaptive workspace bound (mr_bind_adaptive_workspace)");
+    if (ctx->failed) return fail(ctx, MR_ERR_NUMERIC, "mr_step_adaptive: context is in the failed state (call mr_set_x)");
+    return ctx->dtype == MR_F64 ? do_adaptive<double>(ctx, t_end, lambda0, dt, op, max_trials, stats, trace_host, trace_cap)
+                                : do_adaptive<float>(ctx, t_end, lambda0, dt, op, max_trials, stats, trace_host, trace_cap);
+}
+
 extern "C" mr_status mr_diagnostics(mr_ctx* ctx, mr_operator op, mr_diag* out)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
@@ -419,6 +690,49 @@ extern "C" mr_status mr_diagnostics(mr_ctx* ctx, mr_operator op, mr_diag* out)
     if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_diagnostics: unknown operator");
     if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_diagnostics: B0 has not been set");
     return ctx->dtype == MR_F64 ? do_diag<double>(ctx, op, out) : do_diag<float>(ctx, op, out);
+}
+
+extern "C" mr_status mr_convexity(mr_ctx* ctx, int32_t* kappa_dev, int64_t* n_concave)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!n_concave) return fail(ctx, MR_ERR_INVALID_ARG, "mr_convexity: null output");
+    dim3 grid, block;
+    node_launch_dims(ctx, grid, block);
+    unsigned long long* cnt = reinterpret_cast<unsigned long long*>(ctx->diag_out());
+    MR_CUDA(ctx, cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), ctx->stream));
+    if (ctx->dtype == MR_F64)
+        k_convexity<double><<<grid, block, 0, ctx->stream>>>(static_cast<const double*>(ctx->xi(ctx->cur)), grid_params<double>(ctx), kappa_dev, cnt);
+    else
+        k_convexity<float><<<grid, block, 0, ctx->stream>>>(static_cast<const float*>(ctx->xi(ctx->cur)), grid_params<float>(ctx), kappa_dev, cnt);
+    ctx->launches++;
+    MR_CUDA(ctx, cudaGetLastError());
+    unsigned long long r = 0;
+    MR_CUDA(ctx, cudaMemcpyAsync(&r, cnt, sizeof(r), cudaMemcpyDeviceToHost, ctx->stream));
+    MR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *n_concave = (int64_t)r;
+    return MR_OK;
+}
+
+extern "C" mr_status mr_eps_star(mr_ctx* ctx, mr_operator op, int32_t ic, int32_t jc, double a_r, double* alpha_host, double* eps_star)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!eps_star) return fail(ctx, MR_ERR_INVALID_ARG, "mr_eps_star: null output");
+    if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_eps_star: unknown operator");
+    if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_eps_star: B0 has not been set");
+    const bool in_x = ctx->per[0] ? (ic >= 0 && ic < ctx->grid.nx) : (ic > 0 && ic < ctx->grid.nx - 1);
+    const bool in_y = ctx->per[1] ? (jc >= 0 && jc < ctx->grid.ny) : (jc > 0 && jc < ctx->grid.ny - 1);
+    if (!in_x || !in_y) return fail(ctx, MR_ERR_INVALID_ARG, "mr_eps_star: the line (ic, jc, .) must consist of inner nodes");
+    return ctx->dtype == MR_F64 ? do_eps_star<double>(ctx, op, ic, jc, a_r, alpha_host, eps_star)
+                                : do_eps_star<float>(ctx, op, ic, jc, a_r, alpha_host, eps_star);
+}
+
+extern "C" mr_status mr_sigma(mr_ctx* ctx, const void* x_ref_dev, const void* B_ref_dev, double* sigma_x, double* sigma_B)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!x_ref_dev || !B_ref_dev || !sigma_x || !sigma_B) return fail(ctx, MR_ERR_INVALID_ARG, "mr_sigma: null pointer");
+    if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_sigma: B0 has not been set");
+    return ctx->dtype == MR_F64 ? do_sigma<double>(ctx, x_ref_dev, B_ref_dev, sigma_x, sigma_B)
+                                : do_sigma<float>(ctx, x_ref_dev, B_ref_dev, sigma_x, sigma_B);
 }
 
 extern "C" mr_status mr_get_fields(mr_ctx* ctx, mr_operator op, void* x_dev, void* B_dev, void* J_dev)
@@ -430,10 +744,12 @@ extern "C" mr_status mr_get_fields(mr_ctx* ctx, mr_operator op, void* x_dev, voi
     return ctx->dtype == MR_F64 ? do_fields<double>(ctx, op, x_dev, B_dev, J_dev) : do_fields<float>(ctx, op, x_dev, B_dev, J_dev);
 }
 
+/* the host variant synchronises anyway, so it also reports a folded grid (the device variant is asynchronous and does not) */
 extern "C" mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_host, void* B_host, void* J_host)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
     void* outs[3] = { x_host, B_host, J_host };
+    MR_CUDA(ctx, cudaMemsetAsync(ctx->flag(), 0, sizeof(int), ctx->stream));
     for (int w = 0; w < 3; ++w) {
         if (!outs[w]) continue;
         mr_status s = mr_get_fields(ctx, op, w == 0 ? ctx->stage() : nullptr, w == 1 ? ctx->stage() : nullptr,
@@ -441,7 +757,10 @@ extern "C" mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_hos
         if (s != MR_OK) return s;
         MR_CUDA(ctx, cudaMemcpyAsync(outs[w], ctx->stage(), ctx->dense_bytes(), cudaMemcpyDeviceToHost, ctx->stream));
     }
-    MR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    int f = 0;
+    mr_status st = read_flag(ctx, &f);
+    if (st != MR_OK) return st;
+    if (f & FLAG_NUMERIC) return fail(ctx, MR_ERR_NUMERIC, "mr_get_fields_host: det(dx/dX) <= 0 or a non-finite value was met");
     return MR_OK;
 }
 

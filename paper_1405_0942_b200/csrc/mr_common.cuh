@@ -23,17 +23,54 @@ struct GridP {
     long long plane;      // pitch * ny
     long long comp;       // plane * nz (stride between components)
     T twoh[3];            // 2 h_a
+    int per[3];           // 1 = periodic axis (Eqs. 2.12-2.14): in the displacement xi = x - X the ghost nodes of the paper
+                          // are a plain wrap of the index (X itself carries the shift by the period n_a h_a), 0 = line-tied
 };
+
+// is (i,j,k) an inner point along every axis (not on a line-tied face)?  Periodic axes have no faces.
+template <typename T>
+__device__ __forceinline__ bool inner_node(const GridP<T>& g, int i, int j, int k)
+{
+    return (g.per[0] || (i > 0 && i < g.nx - 1)) && (g.per[1] || (j > 0 && j < g.ny - 1)) && (g.per[2] || (k > 0 && k < g.nz - 1));
+}
+
+// element offsets of the +1 / -1 neighbours along the three axes (index wrapped on a periodic axis)
+struct Nbr {
+    long long p[3], m[3];
+};
+template <typename T>
+__device__ __forceinline__ Nbr neighbours(const GridP<T>& g, int i, int j, int k)
+{
+    Nbr q;
+    const long long s[3] = { 1LL, (long long)g.pitch, g.plane };
+    const int idx[3] = { i, j, k }, n[3] = { g.nx, g.ny, g.nz };
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        q.p[a] = (g.per[a] && idx[a] == n[a] - 1) ? -(long long)(n[a] - 1) * s[a] : s[a];
+        q.m[a] = (g.per[a] && idx[a] == 0) ? (long long)(n[a] - 1) * s[a] : -s[a];
+    }
+    return q;
+}
 
 enum : int { FLAG_NUMERIC = 1, FLAG_BOUNDARY = 2 };
 
 // un-normalised first difference (2 h_a d/dX_a) of f along an axis with element stride s, at index idx of n
-template <typename T>
-__device__ __forceinline__ T delta_axis(const T* __restrict__ f, long long p, long long s, int idx, int n)
+// (S = storage type of the field, T = arithmetic type: mr_get_fields evaluates an fp32 state in fp64)
+template <typename T, typename S>
+__device__ __forceinline__ T delta_axis(const S* __restrict__ f, long long p, long long s, int idx, int n)
 {
-    if (idx == 0) return T(4) * f[p + s] - T(3) * f[p] - f[p + 2 * s];
-    if (idx == n - 1) return T(3) * f[p] - T(4) * f[p - s] + f[p - 2 * s];
-    return f[p + s] - f[p - s];
+    if (idx == 0) return T(4) * (T)f[p + s] - T(3) * (T)f[p] - (T)f[p + 2 * s];
+    if (idx == n - 1) return T(3) * (T)f[p] - T(4) * (T)f[p - s] + (T)f[p - 2 * s];
+    return (T)f[p + s] - (T)f[p - s];
+}
+
+// ... with the neighbour offsets sp / sm of this node (periodic axis: central difference through the wrap)
+template <typename T, typename S>
+__device__ __forceinline__ T delta_axis(const S* __restrict__ f, long long p, long long sp, long long sm, int idx, int n, bool per)
+{
+    if (!per && idx == 0) return T(4) * (T)f[p + sp] - T(3) * (T)f[p] - (T)f[p + 2 * sp];
+    if (!per && idx == n - 1) return T(3) * (T)f[p] - T(4) * (T)f[p + sm] + (T)f[p + 2 * sm];
+    return (T)f[p + sp] - (T)f[p + sm];
 }
 
 template <typename T>
@@ -46,29 +83,30 @@ __device__ __forceinline__ T det3(const T (&m)[3][3])
 }
 
 // dF[c][a] at node (i,j,k) from global memory (any node, faces included)
-template <typename T>
-__device__ __forceinline__ void node_dF(const T* __restrict__ xi, const GridP<T>& g, int i, int j, int k, T (&dF)[3][3])
+template <typename T, typename S>
+__device__ __forceinline__ void node_dF(const S* __restrict__ xi, const GridP<T>& g, int i, int j, int k, T (&dF)[3][3])
 {
     const long long p = (long long)k * g.plane + (long long)j * g.pitch + i;
+    const Nbr q = neighbours(g, i, j, k);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const T* f = xi + c * g.comp;
-        dF[c][0] = delta_axis(f, p, 1LL, i, g.nx);
-        dF[c][1] = delta_axis(f, p, (long long)g.pitch, j, g.ny);
-        dF[c][2] = delta_axis(f, p, g.plane, k, g.nz);
+        const S* f = xi + c * g.comp;
+        dF[c][0] = delta_axis<T>(f, p, q.p[0], q.m[0], i, g.nx, g.per[0] != 0);
+        dF[c][1] = delta_axis<T>(f, p, q.p[1], q.m[1], j, g.ny, g.per[1] != 0);
+        dF[c][2] = delta_axis<T>(f, p, q.p[2], q.m[2], k, g.nz, g.per[2] != 0);
         dF[c][c] += g.twoh[c];
     }
 }
 
 // B and D = det dF at node (i,j,k) from global memory
-template <typename T>
-__device__ __forceinline__ void node_B(const T* __restrict__ xi, const T* __restrict__ b, const GridP<T>& g,
+template <typename T, typename S>
+__device__ __forceinline__ void node_B(const S* __restrict__ xi, const S* __restrict__ b, const GridP<T>& g,
                                        int i, int j, int k, T (&B)[3], T& D)
 {
     T dF[3][3];
     node_dF(xi, g, i, j, k, dF);
     const long long p = (long long)k * g.plane + (long long)j * g.pitch + i;
-    const T b0 = b[p], b1 = b[g.comp + p], b2 = b[2 * g.comp + p];
+    const T b0 = (T)b[p], b1 = (T)b[g.comp + p], b2 = (T)b[2 * g.comp + p];
     D = det3(dF);
     const T inv = T(1) / D;
 #pragma unroll
@@ -93,8 +131,8 @@ __device__ __forceinline__ void mimetic_J(const T (&dF)[3][3], const T (&dB)[3][
 }
 
 // Mimetic J at an INTERIOR node, everything from global memory (generic path: B recomputed at the 6 neighbours).
-template <typename T>
-__device__ __forceinline__ void node_J_mimetic(const T* __restrict__ xi, const T* __restrict__ b, const GridP<T>& g,
+template <typename T, typename S>
+__device__ __forceinline__ void node_J_mimetic(const S* __restrict__ xi, const S* __restrict__ b, const GridP<T>& g,
                                                int i, int j, int k, T (&J)[3], T (&B)[3], T& D, bool& bad)
 {
     T dF[3][3];
@@ -103,17 +141,20 @@ __device__ __forceinline__ void node_J_mimetic(const T* __restrict__ xi, const T
     D = det3(dF);
     const T inv = T(1) / D;
     {
-        const T b0 = b[p], b1 = b[g.comp + p], b2 = b[2 * g.comp + p];
+        const T b0 = (T)b[p], b1 = (T)b[g.comp + p], b2 = (T)b[2 * g.comp + p];
 #pragma unroll
         for (int c = 0; c < 3; ++c) B[c] = (dF[c][0] * b0 + dF[c][1] * b1 + dF[c][2] * b2) * inv;
     }
     T dB[3][3];
-    const int di[3] = { 1, 0, 0 }, dj[3] = { 0, 1, 0 }, dk[3] = { 0, 0, 1 };
+    const int n[3] = { g.nx, g.ny, g.nz };
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         T Bp[3], Bm[3], Dp, Dm;
-        node_B(xi, b, g, i + di[a], j + dj[a], k + dk[a], Bp, Dp);
-        node_B(xi, b, g, i - di[a], j - dj[a], k - dk[a], Bm, Dm);
+        int ip[3] = { i, j, k }, im[3] = { i, j, k };
+        ip[a] = ip[a] + 1 == n[a] ? 0 : ip[a] + 1;             // only an inner node comes here: a wrap means a periodic axis
+        im[a] = im[a] == 0 ? n[a] - 1 : im[a] - 1;
+        node_B(xi, b, g, ip[0], ip[1], ip[2], Bp, Dp);
+        node_B(xi, b, g, im[0], im[1], im[2], Bm, Dm);
         bad = bad || !(Dp > T(0)) || !(Dm > T(0));
 #pragma unroll
         for (int c = 0; c < 3; ++c) dB[a][c] = Bp[c] - Bm[c];
@@ -126,25 +167,25 @@ __device__ __forceinline__ void node_J_mimetic(const T* __restrict__ xi, const T
 // un-normalised second differences W[c][q][a] = 4 h_q h_a d2x_c/dX_q dX_a and g[q][a] = delta_a b_q:
 //   Nt[c][a] = W[c][q][a] b_q + dF[c][q] g[q][a],  t[a] = adj[q][c] W[c][q][a]  (= delta_a D, Jacobi),
 //   Q[c][a]  = Nt[c][a] - B_c t[a],   dB_c/dx_m = Q[c][a] adj[a][m] / D^2,   J_l = eps_lmc dB_c/dx_m.
-template <typename T>
-__device__ __forceinline__ void node_J_direct(const T* __restrict__ xi, const T* __restrict__ b, const GridP<T>& g,
+template <typename T, typename S>
+__device__ __forceinline__ void node_J_direct(const S* __restrict__ xi, const S* __restrict__ b, const GridP<T>& g,
                                               int i, int j, int k, T (&J)[3], T (&B)[3], T& D, bool& bad)
 {
     T dF[3][3];
     node_dF(xi, g, i, j, k, dF);
     const long long p = (long long)k * g.plane + (long long)j * g.pitch + i;
-    const long long s[3] = { 1LL, (long long)g.pitch, g.plane };
+    const Nbr nb = neighbours(g, i, j, k);
     T W[3][3][3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const T* f = xi + c * g.comp;
-        const T f0 = f[p];
+        const S* f = xi + c * g.comp;
+        const T f0 = (T)f[p];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            W[c][a][a] = T(4) * (f[p + s[a]] - T(2) * f0 + f[p - s[a]]);
+            W[c][a][a] = T(4) * ((T)f[p + nb.p[a]] - T(2) * f0 + (T)f[p + nb.m[a]]);
 #pragma unroll
             for (int q = a + 1; q < 3; ++q) {
-                const T m = f[p + s[a] + s[q]] - f[p + s[a] - s[q]] - f[p - s[a] + s[q]] + f[p - s[a] - s[q]];
+                const T m = (T)f[p + nb.p[a] + nb.p[q]] - (T)f[p + nb.p[a] + nb.m[q]] - (T)f[p + nb.m[a] + nb.p[q]] + (T)f[p + nb.m[a] + nb.m[q]];
                 W[c][a][q] = m;
                 W[c][q][a] = m;
             }
@@ -153,10 +194,10 @@ __device__ __forceinline__ void node_J_direct(const T* __restrict__ xi, const T*
     T bb[3], gq[3][3];
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
-        const T* f = b + q * g.comp;
-        bb[q] = f[p];
+        const S* f = b + q * g.comp;
+        bb[q] = (T)f[p];
 #pragma unroll
-        for (int a = 0; a < 3; ++a) gq[q][a] = f[p + s[a]] - f[p - s[a]];
+        for (int a = 0; a < 3; ++a) gq[q][a] = (T)f[p + nb.p[a]] - (T)f[p + nb.m[a]];
     }
     // adjugate: adj[a][m] = D * (dF^-1)[a][m]
     T adj[3][3];

@@ -114,12 +114,15 @@ __device__ __forceinline__ void direct_J_smem(const T* __restrict__ xm, const T*
     J[2] = (G(1, 0) - G(0, 1)) * inv2;
 }
 
-template <typename T, int TY, int R>
+// MODE (mr_sym.cuh): MODE_STEP xi+ = xi + dtg J x B;  MODE_RHS out = dtg J x B;  MODE_DIAG the reduction S6 (one
+// DiagPartial per CTA into `out`)
+template <typename T, int TY, int R, int MODE>
 __global__ void __launch_bounds__(TY * 32, 1)
 k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, T* __restrict__ out,
               const StreamArgs<T> a)
 {
     using L = DirectLayout<T, TY, R>;
+    constexpr bool DIAG = MODE == 1, RHS = MODE == 2;
     constexpr int TX = L::TX, BW = L::BW, CS = L::CS, NTH = L::NTHREADS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned char* smem = smem_raw + ((128u - (ptx::smem_u32(smem_raw) & 127u)) & 127u);
@@ -163,6 +166,8 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
 
     bool bad = false;
     T* po = out + (long long)k0 * a.plane + (long long)gj * a.pitch + gi;
+    DiagPartial acc = { 0.0, 0.0, 0.0, INFINITY };          // DIAG: this thread's partial over its INNER nodes (zeta = 1); the
+                                                            // nodes on the line-tied faces are left to k_diag_faces
     int sm = (k0 - 1 - pfirst + R) % R, sc = (k0 - pfirst) % R, sp = (k0 + 1 - pfirst) % R;   // slots of k-1, k, k+1
     uint32_t parp = (uint32_t)(((k0 + 1 - pfirst) / R) & 1);
     int gen = 0;                                                       // named barrier of this iteration (k - k0) % R
@@ -171,18 +176,27 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
         if (k + 1 <= plast) ptx::mbar_wait(bar + 8u * (uint32_t)sp, parp);
         const T* xc = sx + sc * L::SLOT + o;
         T x[3] = { xc[0], xc[CS], xc[2 * CS] };
-        if (in_xy && k > 0 && k < nz - 1) {
+        if (RHS) x[0] = x[1] = x[2] = T(0);
+        const bool inner = in_xy && k > 0 && k < nz - 1;
+        if (inner) {
             T J[3], B[3], u[3], D;
             direct_J_smem<T, BW, CS>(sx + sm * L::SLOT + o, xc, sx + sp * L::SLOT + o, sb + sm * L::SLOT + o, sb + sc * L::SLOT + o,
                                      sb + sp * L::SLOT + o, twoh, J, B, D, bad);
             cross3(J, B, u);
+            if constexpr (DIAG) {
+                const double b2 = (double)B[0] * B[0] + (double)B[1] * B[1] + (double)B[2] * B[2];
+                const double fm = sqrt((double)u[0] * u[0] + (double)u[1] * u[1] + (double)u[2] * u[2]);
+                DiagPartial v = { b2 * (double)D, fm, fm / b2, (double)D };
+                diag_combine(acc, v);
+            } else {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                x[c] += a.dtg * u[c];
-                bad = bad || !(fabs(x[c]) < T(1e30));
+                for (int c = 0; c < 3; ++c) {
+                    x[c] += a.dtg * u[c];
+                    bad = bad || !(fabs(x[c]) < T(1e30));
+                }
             }
         }
-        if (in_dom) {
+        if (!DIAG && in_dom) {
             po[0] = x[0];
             po[a.comp] = x[1];
             po[2 * a.comp] = x[2];
@@ -198,6 +212,26 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
         if (++gen == R) gen = 0;
         sm = sc; sc = sp;
         if (++sp == R) { sp = 0; parp ^= 1u; }
+    }
+    if constexpr (DIAG) {
+        __syncthreads();                                    // the ring is drained: shared memory is free
+#pragma unroll
+        for (int o2 = 16; o2 > 0; o2 >>= 1) {
+            DiagPartial w;
+            w.e = __shfl_down_sync(0xffffffffu, acc.e, o2);
+            w.fmax = __shfl_down_sync(0xffffffffu, acc.fmax, o2);
+            w.xi = __shfl_down_sync(0xffffffffu, acc.xi, o2);
+            w.dmin = __shfl_down_sync(0xffffffffu, acc.dmin, o2);
+            diag_combine(acc, w);
+        }
+        DiagPartial* shp = reinterpret_cast<DiagPartial*>(smem);
+        if (lane == 0) shp[warp] = acc;
+        __syncthreads();
+        if (tid == 0) {
+            DiagPartial v = shp[0];
+            for (int w = 1; w < TY; ++w) diag_combine(v, shp[w]);
+            reinterpret_cast<DiagPartial*>(out)[blockIdx.x] = v;
+        }
     }
     if (bad) atomicOr(a.flag, FLAG_NUMERIC);
 }
@@ -227,8 +261,17 @@ inline bool build_direct_plan(StreamPlan* p, const StreamGeom& g, bool f64, void
     p->tiles_x = (g.nx + Ld::TX - 1) / Ld::TX;
     p->tiles_y = (g.ny + kXTY - 1) / kXTY;
     p->smem_bytes = f64 ? Ld::BYTES : Lf::BYTES;
-    cudaError_t e = f64 ? cudaFuncSetAttribute(k_step_direct<double, kXTY, kXR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes)
-                        : cudaFuncSetAttribute(k_step_direct<float, kXTY, kXR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes);
+    cudaError_t e = cudaSuccess;
+    const int sb = (int)p->smem_bytes;
+    if (f64) {
+        e = cudaFuncSetAttribute(k_step_direct<double, kXTY, kXR, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_direct<double, kXTY, kXR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_direct<double, kXTY, kXR, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+    } else {
+        e = cudaFuncSetAttribute(k_step_direct<float, kXTY, kXR, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_direct<float, kXTY, kXR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_direct<float, kXTY, kXR, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+    }
     if (e != cudaSuccess) {
         *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
         return false;
@@ -238,10 +281,17 @@ inline bool build_direct_plan(StreamPlan* p, const StreamGeom& g, bool f64, void
     return true;
 }
 
-template <typename T>
-inline cudaError_t launch_direct_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream)
+inline bool direct_bind_stage(StreamPlan* p, void* xs)
 {
-    using L = DirectLayout<T, kXTY, kXR>;
+    const int bw = p->f64 ? DirectLayout<double, kXTY, kXR>::BW : DirectLayout<float, kXTY, kXR>::BW;
+    if (!encode_map(&p->map_xi[2], p->f64, xs, p->g, bw, kXTY + 2)) return false;
+    p->xi[2] = xs;
+    return true;
+}
+
+template <typename T>
+inline StreamArgs<T> direct_args(const StreamPlan& p, T dtg, int* flag)
+{
     StreamArgs<T> a;
     a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
     a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
@@ -251,8 +301,30 @@ inline cudaError_t launch_direct_step(const StreamPlan& p, int cur, T dtg, int* 
     a.ntiles = p.tiles_x * p.tiles_y;
     a.chunk_len = p.chunk_len;
     a.flag = flag;
+    return a;
+}
+
+// one step / one right-hand side of the state in the plan's buffer `cur` (see launch_sym_step)
+template <typename T>
+inline cudaError_t launch_direct_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream, bool rhs = false, void* out = nullptr)
+{
+    using L = DirectLayout<T, kXTY, kXR>;
+    const StreamArgs<T> a = direct_args<T>(p, dtg, flag);
+    T* o = static_cast<T*>(out ? out : p.xi[1 - cur]);
     const int grid = a.ntiles * p.nchunks;
-    k_step_direct<T, kXTY, kXR><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, static_cast<T*>(p.xi[1 - cur]), a);
+    if (rhs) k_step_direct<T, kXTY, kXR, 2><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, o, a);
+    else k_step_direct<T, kXTY, kXR, 0><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, o, a);
+    return cudaGetLastError();
+}
+
+// S6 over the INNER nodes by the same pass: one DiagPartial per CTA into partials[0 .. *nblocks)
+template <typename T>
+inline cudaError_t launch_direct_diag(const StreamPlan& p, int cur, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
+{
+    using L = DirectLayout<T, kXTY, kXR>;
+    const StreamArgs<T> a = direct_args<T>(p, (T)0, flag);
+    *nblocks = a.ntiles * p.nchunks;
+    k_step_direct<T, kXTY, kXR, 1><<<*nblocks, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();
 }
 

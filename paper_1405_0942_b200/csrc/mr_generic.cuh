@@ -34,7 +34,7 @@ __global__ void k_import_x(const T* __restrict__ x, T* __restrict__ xi, GridP<T>
     const long long N = (long long)g.nx * g.ny * g.nz;
     const long long q = ((long long)k * g.ny + j) * g.nx + i;
     const long long p = (long long)k * g.plane + (long long)j * g.pitch + i;
-    const bool bnd = i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1;
+    const bool bnd = !inner_node(g, i, j, k);
     const int idx[3] = { i, j, k };
     bool off = false;
 #pragma unroll
@@ -52,6 +52,43 @@ __global__ void k_import_x(const T* __restrict__ x, T* __restrict__ xi, GridP<T>
     if (off) atomicOr(flag, FLAG_BOUNDARY);
 }
 
+// xi (dense) -> xi (padded): the displacement itself crosses the ABI (on an fp32 context x = X + xi would lose
+// eps |X| per node, 300 times the rounding of xi).  Nodes on a line-tied face must have xi = 0, else FLAG_BOUNDARY.
+template <typename T>
+__global__ void k_import_xi(const T* __restrict__ src, T* __restrict__ xi, GridP<T> g, int* __restrict__ flag)
+{
+    int i, j, k;
+    if (!node_of_thread(g.nx, g.ny, g.nz, i, j, k)) return;
+    const long long N = (long long)g.nx * g.ny * g.nz;
+    const long long q = ((long long)k * g.ny + j) * g.nx + i;
+    const long long p = (long long)k * g.plane + (long long)j * g.pitch + i;
+    const bool bnd = !inner_node(g, i, j, k);
+    bool off = false;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        T v = src[c * N + q];
+        if (bnd) {
+            if (!(fabs((double)v) <= 1e-6 * 0.5 * (double)g.twoh[c])) off = true;
+            v = T(0);
+        }
+        xi[c * g.comp + p] = v;
+    }
+    if (off) atomicOr(flag, FLAG_BOUNDARY);
+}
+
+// padded field (xi, or a velocity) -> dense caller buffer
+template <typename T>
+__global__ void k_export_padded(const T* __restrict__ src, T* __restrict__ dst, GridP<T> g)
+{
+    int i, j, k;
+    if (!node_of_thread(g.nx, g.ny, g.nz, i, j, k)) return;
+    const long long N = (long long)g.nx * g.ny * g.nz;
+    const long long q = ((long long)k * g.ny + j) * g.nx + i;
+    const long long p = (long long)k * g.plane + (long long)j * g.pitch + i;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dst[c * N + q] = src[c * g.comp + p];
+}
+
 // B0 (dense) -> b_a = scale_a * B0_a (padded), scale_a = 4 h_b h_c
 template <typename T>
 __global__ void k_import_B0(const T* __restrict__ B0, T* __restrict__ b, GridP<T> g, double s0, double s1, double s2)
@@ -66,9 +103,12 @@ __global__ void k_import_B0(const T* __restrict__ B0, T* __restrict__ b, GridP<T
     b[2 * g.comp + p] = (T)((double)B0[2 * N + q] * s2);
 }
 
-// Materialise x = X + xi, B (all nodes) and J (interior, 0 on the boundary) into dense caller buffers.
+// Materialise x = X + xi, B (all nodes) and J (interior, 0 on the boundary) into dense caller buffers.  The fields are
+// evaluated in fp64 whatever the storage type T of the state is and rounded to T at the end: on an fp32 context they
+// are then as accurate as the fp32 STATE allows (J formed in fp32 arithmetic carries eps |B| / (2h |grad B|), about 1.2e-5
+// of max |J| at h = 8/511, reading Q15); the step kernels themselves compute in T.
 template <typename T, int OP>
-__global__ void k_fields(const T* __restrict__ xi, const T* __restrict__ b, GridP<T> g, DomainP d,
+__global__ void k_fields(const T* __restrict__ xi, const T* __restrict__ b, GridP<double> g, DomainP d,
                          T* __restrict__ x_out, T* __restrict__ B_out, T* __restrict__ J_out, int* __restrict__ flag)
 {
     int i, j, k;
@@ -82,12 +122,12 @@ __global__ void k_fields(const T* __restrict__ xi, const T* __restrict__ b, Grid
         for (int c = 0; c < 3; ++c) x_out[c * N + q] = (T)__dadd_rn(ref_coord(d.lo[c], d.h[c], idx[c]), (double)xi[c * g.comp + p]);
     }
     if (!B_out && !J_out) return;
-    const bool bnd = i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1;
-    T B[3], J[3] = { T(0), T(0), T(0) }, D;
+    const bool bnd = !inner_node(g, i, j, k);
+    double B[3], J[3] = { 0.0, 0.0, 0.0 }, D;
     bool bad = false;
     if (bnd || !J_out) {
         node_B(xi, b, g, i, j, k, B, D);
-        bad = !(D > T(0));
+        bad = !(D > 0.0);
     } else if (OP == 0) {
         node_J_mimetic(xi, b, g, i, j, k, J, B, D, bad);
     } else {
@@ -96,13 +136,14 @@ __global__ void k_fields(const T* __restrict__ xi, const T* __restrict__ b, Grid
     if (bad) atomicOr(flag, FLAG_NUMERIC);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        if (B_out) B_out[c * N + q] = B[c];
-        if (J_out) J_out[c * N + q] = J[c];
+        if (B_out) B_out[c * N + q] = (T)B[c];
+        if (J_out) J_out[c * N + q] = (T)J[c];
     }
 }
 
 // Generic fused step: xi_out = xi_in + dtg * J x B on interior nodes, copy on boundary nodes (S1-S5).
-template <typename T, int OP>
+// RHS = true: xi_out = dtg * J x B instead (the velocity u = gamma J x B with dtg = gamma; 0 on boundary nodes).
+template <typename T, int OP, bool RHS = false>
 __global__ void __launch_bounds__(256)
 k_step_generic(const T* __restrict__ xi_in, T* __restrict__ xi_out, const T* __restrict__ b, GridP<T> g, T dtg,
                int* __restrict__ flag)
@@ -110,8 +151,9 @@ k_step_generic(const T* __restrict__ xi_in, T* __restrict__ xi_out, const T* __r
     int i, j, k;
     if (!node_of_thread(g.nx, g.ny, g.nz, i, j, k)) return;
     const long long p = (long long)k * g.plane + (long long)j * g.pitch + i;
-    const bool bnd = i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1;
+    const bool bnd = !inner_node(g, i, j, k);
     T o[3] = { xi_in[p], xi_in[g.comp + p], xi_in[2 * g.comp + p] };
+    if (RHS) o[0] = o[1] = o[2] = T(0);
     if (!bnd) {
         T B[3], J[3], u[3], D;
         bool bad = false;
@@ -180,7 +222,7 @@ k_diag(const T* __restrict__ xi, const T* __restrict__ b, GridP<T> g, DiagPartia
     for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
         const int j = (int)(r % g.ny), k = (int)(r / g.ny);
         for (int i = threadIdx.x; i < g.nx; i += blockDim.x) {
-            const bool bnd = i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1;
+            const bool bnd = !inner_node(g, i, j, k);
             T B[3], J[3], D;
             if (bnd) {
                 node_B(xi, b, g, i, j, k, B, D);
@@ -191,9 +233,9 @@ k_diag(const T* __restrict__ xi, const T* __restrict__ b, GridP<T> g, DiagPartia
             }
             const double b2 = (double)B[0] * B[0] + (double)B[1] * B[1] + (double)B[2] * B[2];
             double zeta = 1.0;
-            if (i == 0 || i == g.nx - 1) zeta *= 0.5;
-            if (j == 0 || j == g.ny - 1) zeta *= 0.5;
-            if (k == 0 || k == g.nz - 1) zeta *= 0.5;
+            if (!g.per[0] && (i == 0 || i == g.nx - 1)) zeta *= 0.5;
+            if (!g.per[1] && (j == 0 || j == g.ny - 1)) zeta *= 0.5;
+            if (!g.per[2] && (k == 0 || k == g.nz - 1)) zeta *= 0.5;
             DiagPartial v = { zeta * b2 * (double)D, 0.0, 0.0, (double)D };
             if (!bnd) {
                 T f[3];
@@ -202,6 +244,40 @@ k_diag(const T* __restrict__ xi, const T* __restrict__ b, GridP<T> g, DiagPartia
                 v.fmax = fm;
                 v.xi = fm / b2;
             }
+            diag_combine(acc, v);
+        }
+    }
+    if (bad) atomicOr(flag, FLAG_NUMERIC);
+    acc = diag_block_reduce(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+}
+
+// S6 contributions of the nodes on line-tied faces only (zeta |B|^2 D and min D; they carry no J): the complement of the
+// streaming pass of the direct operator, which reduces the inner nodes.  Same row ownership and order as k_diag.
+template <typename T>
+__global__ void __launch_bounds__(128)
+k_diag_faces(const T* __restrict__ xi, const T* __restrict__ b, GridP<T> g, DiagPartial* __restrict__ partials, int* __restrict__ flag)
+{
+    DiagPartial acc = { 0.0, 0.0, 0.0, INFINITY };
+    const long long rows = (long long)g.ny * g.nz;
+    bool bad = false;
+    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
+        const int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        const bool face_row = (!g.per[1] && (j == 0 || j == g.ny - 1)) || (!g.per[2] && (k == 0 || k == g.nz - 1));
+        if (!face_row && g.per[0]) continue;
+        const int cnt = face_row ? g.nx : 2;                 // the whole row, or its two end nodes
+        for (int q = threadIdx.x; q < cnt; q += blockDim.x) {
+            const int i = face_row ? q : (q == 0 ? 0 : g.nx - 1);
+            if (inner_node(g, i, j, k)) continue;
+            T B[3], D;
+            node_B(xi, b, g, i, j, k, B, D);
+            bad = bad || !(D > T(0));
+            const double b2 = (double)B[0] * B[0] + (double)B[1] * B[1] + (double)B[2] * B[2];
+            double zeta = 1.0;
+            if (!g.per[0] && (i == 0 || i == g.nx - 1)) zeta *= 0.5;
+            if (!g.per[1] && (j == 0 || j == g.ny - 1)) zeta *= 0.5;
+            if (!g.per[2] && (k == 0 || k == g.nz - 1)) zeta *= 0.5;
+            DiagPartial v = { zeta * b2 * (double)D, 0.0, 0.0, (double)D };
             diag_combine(acc, v);
         }
     }

@@ -39,9 +39,9 @@ struct StreamPlan {
     const char* name = "stream";
     std::string why;
     StreamGeom g{};
-    CUtensorMap map_xi[2];
+    CUtensorMap map_xi[3];      // the two state buffers and, once bound, the stage buffer of the adaptive integrator
     CUtensorMap map_b;
-    void* xi[2] = { nullptr, nullptr };
+    void* xi[3] = { nullptr, nullptr, nullptr };
     const void* b = nullptr;
     int tiles_x = 0, tiles_y = 0, nchunks = 0, chunk_len = 0;
     size_t smem_bytes = 0;

@@ -63,13 +63,16 @@ struct SymLayout {
 
 template <int Q> using Phase = std::integral_constant<int, Q>;
 
-template <typename T, bool DIAG>
+enum : int { MODE_STEP = 0, MODE_DIAG = 1, MODE_RHS = 2 };     // xi+ = xi + dt u  |  the reduction S6  |  out = u = gamma J x B
+
+template <typename T, int MODE>
 __global__ void __maxnreg__(96)
 k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, const T* __restrict__ in,
            T* __restrict__ out, const StreamArgs<T> a)
 {
     using L = SymLayout<T>;
     using W32 = tmem::Words<T>;
+    constexpr bool DIAG = MODE == MODE_DIAG, RHS = MODE == MODE_RHS;
     constexpr int TX = L::TX, TY = L::TY, NTW = L::NTW, BW = L::BW, CSX = L::CSX, CSB = L::CSB, BBW = L::BBW, BCS = L::BCS;
     constexpr int NW = L::NWARPS, WN = L::WN, C0W = L::C0W, C1W = L::C1W, REC = L::REC;
     static_assert(L::TMEM_COLS == 256 || L::TMEM_COLS == 128, "TMEM columns: a power of two");
@@ -228,10 +231,11 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 #pragma unroll
                     for (int c = 0; c < 3; ++c) dF[c][2] = T(4) * f2[c * CSX] - T(3) * x1[c] - f3[c * CSX];
                 }
-                if (special & 32u) {            // top face: 3 x(nz-1) - 4 x(nz-2) + x(nz-3); the plane nz-3 is still in its position
-                    const T* fm = px + S2 * L::SLOTX;
+                if (special & 32u) {            // top face: 3 x(nz-1) - 4 x(nz-2) + x(nz-3); the own xi of the plane nz-3 comes from
+                                                // global memory (once per column; a last chunk of one plane never loads that plane)
+                    const long long o3 = (long long)(nz - 3) * a.plane + (long long)gj * a.pitch + gi;
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) dF[c][2] = T(3) * x1[c] - T(4) * xp[c] + fm[c * CSX];
+                    for (int c = 0; c < 3; ++c) dF[c][2] = T(3) * x1[c] - T(4) * xp[c] + (dom ? in[c * a.comp + o3] : T(0));
                 }
                 if (special & 15u) face_fix<T, BW, CSX>(fr, special & 15u, dF);
             }
@@ -337,7 +341,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 #ifdef MR_X_TMEM
                 for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], W32::get(w1 + (4 + c) * WN));
 #else
-                for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], xp[c]);
+                for (int c = 0; c < 3; ++c) x[c] = RHS ? s * uu[c] : fma(s, uu[c], xp[c]);
 #endif
 #ifndef MR_NOXCHK
                 ok = ok && is_finite(x[0] + x[1] + x[2]);
@@ -391,7 +395,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         } else if (st) {
             T* pl = out + (long long)(nz - 1) * a.plane + (long long)gj * a.pitch + gi;
 #pragma unroll
-            for (int c = 0; c < 3; ++c) pl[c * a.comp] = (ql & 1) ? xh[1][c] : xh[0][c];
+            for (int c = 0; c < 3; ++c) pl[c * a.comp] = RHS ? T(0) : (ql & 1) ? xh[1][c] : xh[0][c];
         }
     }
     if (!ok) atomicOr(a.flag, FLAG_NUMERIC);
@@ -446,11 +450,13 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
     cudaError_t e = cudaSuccess;
     const int sb = (int)p->smem_bytes;
     if (f64) {
-        e = cudaFuncSetAttribute(k_step_sym<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        e = cudaFuncSetAttribute(k_step_sym<double, MODE_STEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<double, MODE_DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<double, MODE_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
     } else {
-        e = cudaFuncSetAttribute(k_step_sym<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        e = cudaFuncSetAttribute(k_step_sym<float, MODE_STEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<float, MODE_DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<float, MODE_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
     }
     if (e != cudaSuccess) {
         *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
@@ -458,6 +464,15 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
     }
     choose_chunks(p->tiles_x * p->tiles_y, g.nz, sm_count, &p->nchunks, &p->chunk_len);
     p->usable = true;
+    return true;
+}
+
+// tensor map of the adaptive integrator's stage buffer (same box as the state buffers)
+inline bool sym_bind_stage(StreamPlan* p, void* xs)
+{
+    const int bw = p->f64 ? SymLayout<double>::BW : SymLayout<float>::BW;
+    if (!encode_map(&p->map_xi[2], p->f64, xs, p->g, bw, SymLayout<double>::TY + 4)) return false;
+    p->xi[2] = xs;
     return true;
 }
 
@@ -476,12 +491,19 @@ inline StreamArgs<T> sym_args(const StreamPlan& p, T dtg, int* flag)
     return a;
 }
 
+// One step (rhs = false: out = xi + dtg J x B) or one right-hand side (rhs = true: out = dtg J x B, dtg = gamma) of the
+// state in the plan's buffer `cur` (0, 1: the state buffers; 2: the stage buffer) into the padded field `out`.
 template <typename T>
-inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream)
+inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream, bool rhs = false, void* out = nullptr)
 {
     const StreamArgs<T> a = sym_args<T>(p, dtg, flag);
-    k_step_sym<T, false><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
-        p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), static_cast<T*>(p.xi[1 - cur]), a);
+    T* o = static_cast<T*>(out ? out : p.xi[1 - cur]);
+    if (rhs)
+        k_step_sym<T, MODE_RHS><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+            p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), o, a);
+    else
+        k_step_sym<T, MODE_STEP><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+            p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), o, a);
     return cudaGetLastError();
 }
 
@@ -491,7 +513,7 @@ inline cudaError_t launch_sym_diag(const StreamPlan& p, int cur, DiagPartial* pa
 {
     const StreamArgs<T> a = sym_args<T>(p, (T)0, flag);
     *nblocks = a.ntiles * p.nchunks;
-    k_step_sym<T, true><<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+    k_step_sym<T, MODE_DIAG><<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
         p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();
 }

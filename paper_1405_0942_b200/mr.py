@@ -28,6 +28,7 @@ MR_F64, MR_F32 = 0, 1
 STATUS_NAMES = {0: "MR_OK", 1: "MR_ERR_INVALID_ARG", 2: "MR_ERR_WORKSPACE", 3: "MR_ERR_CUDA", 4: "MR_ERR_STATE",
                 5: "MR_ERR_NUMERIC"}
 OPERATORS = {"mimetic": MR_OP_MIMETIC, "direct": MR_OP_DIRECT}
+BOUNDARIES = {"line_tied": MR_BC_LINE_TIED, "periodic": MR_BC_PERIODIC}
 
 
 class mr_grid(C.Structure):
@@ -43,6 +44,11 @@ class mr_boundary(C.Structure):
                 ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p)]
 
 
+class mr_adapt_stats(C.Structure):
+    _fields_ = [("accepted", C.c_int64), ("rejected", C.c_int64), ("rhs_evals", C.c_int64), ("time", C.c_double),
+                ("dt_next", C.c_double), ("last_lambda", C.c_double)]
+
+
 class mr_diag(C.Structure):
     _fields_ = [("time", C.c_double), ("steps", C.c_int64), ("energy", C.c_double), ("max_jxb", C.c_double),
                 ("xi", C.c_double), ("min_det", C.c_double)]
@@ -55,7 +61,22 @@ lib.mr_create.argtypes = [C.POINTER(mr_grid), C.POINTER(mr_domain), C.POINTER(mr
 lib.mr_create.restype = C.c_int
 lib.mr_destroy.argtypes = [_ctx_p]
 lib.mr_destroy.restype = C.c_int
-for _n in ("mr_set_B0", "mr_set_B0_host", "mr_set_x", "mr_set_x_host"):
+lib.mr_adaptive_workspace_bytes.argtypes = [C.POINTER(mr_grid), C.c_int]
+lib.mr_adaptive_workspace_bytes.restype = C.c_size_t
+lib.mr_bind_adaptive_workspace.argtypes = [_ctx_p, C.c_void_p, C.c_size_t]
+lib.mr_bind_adaptive_workspace.restype = C.c_int
+lib.mr_step_adaptive.argtypes = [_ctx_p, C.c_double, C.c_double, C.POINTER(C.c_double), C.c_int, C.c_int64, C.POINTER(mr_adapt_stats),
+                                 C.c_void_p, C.c_int64]
+lib.mr_step_adaptive.restype = C.c_int
+lib.mr_rhs.argtypes = [_ctx_p, C.c_int, C.c_void_p]
+lib.mr_rhs.restype = C.c_int
+lib.mr_convexity.argtypes = [_ctx_p, C.c_void_p, C.POINTER(C.c_int64)]
+lib.mr_convexity.restype = C.c_int
+lib.mr_eps_star.argtypes = [_ctx_p, C.c_int, C.c_int32, C.c_int32, C.c_double, C.c_void_p, C.POINTER(C.c_double)]
+lib.mr_eps_star.restype = C.c_int
+lib.mr_sigma.argtypes = [_ctx_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+lib.mr_sigma.restype = C.c_int
+for _n in ("mr_set_B0", "mr_set_B0_host", "mr_set_x", "mr_set_x_host", "mr_set_xi", "mr_get_xi"):
     getattr(lib, _n).argtypes = [_ctx_p, C.c_void_p]
     getattr(lib, _n).restype = C.c_int
 lib.mr_step.argtypes = [_ctx_p, C.c_int64, C.c_double, C.c_int]
@@ -109,6 +130,9 @@ class Relaxation:
     def __init__(self, n, lo, hi, dtype="f64", gamma=1.0, bc=("line_tied",) * 3, device="cuda", stream=None):
         import torch
 
+        for b in bc:
+            if b not in BOUNDARIES:
+                raise MrError(MR_ERR_INVALID_ARG, "unknown boundary type %r (expected one of %s)" % (b, sorted(BOUNDARIES)))
         self._torch = torch
         self.n = tuple(int(v) for v in n)
         self.shape = (3, self.n[2], self.n[1], self.n[0])
@@ -124,11 +148,13 @@ class Relaxation:
         if nbytes == 0:
             raise MrError(MR_ERR_INVALID_ARG, "invalid grid %r / dtype %r" % (self.n, dtype))
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            with torch.cuda.stream(self.stream):            # the workspace belongs to the stream the library works on
+                self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._aworkspace = None
             g = mr_grid(*self.n)
             d = mr_domain((C.c_double * 3)(*[float(v) for v in lo]), (C.c_double * 3)(*[float(v) for v in hi]))
-            bcs = (C.c_int * 3)(*[MR_BC_LINE_TIED if b == "line_tied" else MR_BC_PERIODIC for b in bc])
+            bcs = (C.c_int * 3)(*[BOUNDARIES[b] for b in bc])
             b = mr_boundary(bcs, float(gamma), MR_F64 if dtype == "f64" else MR_F32, self.workspace.data_ptr(),
                             nbytes, self.stream.cuda_stream)
             st = lib.mr_create(C.byref(g), C.byref(d), C.byref(b), C.byref(self._ctx))
@@ -147,7 +173,16 @@ class Relaxation:
         if t.device != self.device or t.dtype != self.tdtype or tuple(t.shape) != self.shape or not t.is_contiguous():
             raise MrError(MR_ERR_INVALID_ARG, "%s must be a contiguous %s tensor of shape %r on %s"
                           % (name, self.tdtype, self.shape, self.device))
+        self._order(t)
         return t.data_ptr()
+
+    def _order(self, t):
+        """The library enqueues on its own stream: if the caller's current stream is another one, make ours wait for the
+        work already queued there (the tensor's producer) and tell the allocator that ours uses the tensor."""
+        cur = self._torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            self.stream.wait_stream(cur)
+            t.record_stream(self.stream)
 
     def _host(self, t, name):
         if t is None:
@@ -202,6 +237,74 @@ class Relaxation:
                 self._check(lib.mr_get_fields_host(self._ctx, _op(op), self._host(x, "x"), self._host(B, "B"), self._host(J, "J")))
             else:
                 self._check(lib.mr_get_fields(self._ctx, _op(op), self._dev(x, "x"), self._dev(B, "B"), self._dev(J, "J")))
+
+    def set_xi(self, xi):
+        """mr_set_xi: the displacement x - X (what fp32 contexts should exchange instead of positions)."""
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_set_xi(self._ctx, self._dev(xi, "xi")))
+
+    def get_xi(self):
+        out = self.empty_field()
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_get_xi(self._ctx, self._dev(out, "xi")))
+        return out
+
+    def rhs(self, op="mimetic"):
+        """mr_rhs: the velocity u = gamma J x B of the current state (0 on line-tied boundary nodes)."""
+        out = self.empty_field()
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_rhs(self._ctx, _op(op), self._dev(out, "u")))
+        return out
+
+    def step_adaptive(self, t_end, lambda0, dt, op="mimetic", max_trials=1000000, trace=False):
+        """mr_step_adaptive: returns a dict (accepted, rejected, rhs_evals, time, dt_next, last_lambda[, trace])."""
+        torch = self._torch
+        with torch.cuda.device(self.device):
+            if self._aworkspace is None:
+                g = mr_grid(*self.n)
+                nb = int(lib.mr_adaptive_workspace_bytes(C.byref(g), MR_F64 if self.dtype == "f64" else MR_F32))
+                with torch.cuda.stream(self.stream):
+                    self._aworkspace = torch.empty(nb, dtype=torch.uint8, device=self.device)
+                self._check(lib.mr_bind_adaptive_workspace(self._ctx, self._aworkspace.data_ptr(), nb))
+            st, d = mr_adapt_stats(), C.c_double(float(dt))
+            cap = int(min(max_trials, 100000)) if trace else 0
+            buf = (C.c_double * (4 * cap))() if cap else None
+            rc = lib.mr_step_adaptive(self._ctx, float(t_end), float(lambda0), C.byref(d), _op(op), int(max_trials), C.byref(st),
+                                      C.cast(buf, C.c_void_p) if cap else None, cap)
+        out = {"accepted": st.accepted, "rejected": st.rejected, "rhs_evals": st.rhs_evals, "time": st.time, "dt_next": st.dt_next,
+               "last_lambda": st.last_lambda}
+        if trace:
+            n = st.accepted + st.rejected
+            out["trace"] = [tuple(buf[4 * q:4 * q + 4]) for q in range(min(n, cap))]
+        self.last_adaptive = out
+        self._check(rc)
+        return out
+
+    def convexity(self, want_field=False):
+        """mr_convexity: (number of nodes with kappa = -1, kappa as an int32 tensor (nz, ny, nx) or None)."""
+        torch = self._torch
+        n = C.c_int64()
+        kap = torch.empty(self.shape[1:], dtype=torch.int32, device=self.device) if want_field else None
+        with torch.cuda.device(self.device):
+            if kap is not None:
+                self._order(kap)
+            self._check(lib.mr_convexity(self._ctx, kap.data_ptr() if kap is not None else None, C.byref(n)))
+        return int(n.value), kap
+
+    def eps_star(self, ic, jc, a_r, op="mimetic"):
+        """mr_eps_star: (alpha* along the grid line (ic, jc, .) as a list of nz floats, eps*)."""
+        al = (C.c_double * self.n[2])()
+        e = C.c_double()
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_eps_star(self._ctx, _op(op), int(ic), int(jc), float(a_r), C.cast(al, C.c_void_p), C.byref(e)))
+        return list(al), e.value
+
+    def sigma(self, x_ref, B_ref):
+        """mr_sigma: (sigma_x, sigma_B) against dense device references."""
+        sx, sb = C.c_double(), C.c_double()
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_sigma(self._ctx, self._dev(x_ref, "x_ref"), self._dev(B_ref, "B_ref"), C.byref(sx), C.byref(sb)))
+        return sx.value, sb.value
 
     def set_variant(self, name):
         self._check(lib.mr_set_variant(self._ctx, name.encode()))

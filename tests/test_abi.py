@@ -61,14 +61,31 @@ def test_create_validates_before_any_cuda_call(mr):
     assert _create(mr, hi=(4, -4, 8))[0] == mr.MR_ERR_INVALID_ARG
     assert _create(mr, gamma=0.0)[0] == mr.MR_ERR_INVALID_ARG
     assert _create(mr, dtype=7)[0] == mr.MR_ERR_INVALID_ARG
-    st, ctx, msg = _create(mr, bc=(0, 0, 1))
-    assert st == mr.MR_ERR_INVALID_ARG and "periodic" in msg and not ctx.value
+    st, ctx, msg = _create(mr, bc=(0, 0, 2))
+    assert st == mr.MR_ERR_INVALID_ARG and "boundary" in msg and not ctx.value
     assert _create(mr, ws=None)[0] == mr.MR_ERR_WORKSPACE
     assert _create(mr, ws=264)[0] == mr.MR_ERR_WORKSPACE            # misaligned
     assert _create(mr, ws_bytes=1024)[0] == mr.MR_ERR_WORKSPACE     # too small
 
 
+def test_adaptive_workspace_bytes_is_pure_host_arithmetic(mr):
+    g = mr.mr_grid(256, 256, 512)
+    field = 3 * 256 * 256 * 512 * 8
+    nb = mr.lib.mr_adaptive_workspace_bytes(C.byref(g), mr.MR_F64)
+    assert 7 * field <= nb < 7 * field + (1 << 20)           # six stage velocities and the stage state
+    bad = mr.mr_grid(4, 16, 16)
+    assert mr.lib.mr_adaptive_workspace_bytes(C.byref(bad), mr.MR_F64) == 0
+
+
+def test_binding_rejects_unknown_boundary_names(mr):
+    with pytest.raises(mr.MrError):
+        mr.Relaxation((16, 16, 32), (-4, -4, -8), (4, 4, 8), bc=("line_tied", "open", "line_tied"), device="cuda")
+
+
 def test_null_context_calls_return_invalid_arg(mr):
+    assert mr.lib.mr_step_adaptive(None, 1.0, 1e-6, None, 0, 10, None, None, 0) == mr.MR_ERR_INVALID_ARG
+    assert mr.lib.mr_rhs(None, 0, None) == mr.MR_ERR_INVALID_ARG
+    assert mr.lib.mr_convexity(None, None, None) == mr.MR_ERR_INVALID_ARG
     assert mr.lib.mr_step(None, 1, 0.1, 0) == mr.MR_ERR_INVALID_ARG
     assert mr.lib.mr_set_B0(None, None) == mr.MR_ERR_INVALID_ARG
     assert mr.lib.mr_diagnostics(None, 0, None) == mr.MR_ERR_INVALID_ARG

@@ -1,0 +1,261 @@
+"""GPU parity tests of the SURVEY 8(f) rows: the adaptive Cash-Karp integrator (section 2.4), periodic boundaries
+(Eqs. 2.12-2.14), convexity (Eqs. 3.10-3.11), alpha*/eps* (Eqs. 3.5-3.7), sigma_B/sigma_x (Eqs. 3.8-3.9) and the
+config-3 report at full size -- the CUDA path through the C-ABI against the CPU oracle on the same seeded inputs.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import mro  # noqa: E402  (test infrastructure)
+from paper_1405_0942_b200 import inputs as I  # noqa: E402
+
+from gpu_common import CASES, TOL_100, TOL_STEP, case, dev, fields_np, make_sim, nrel, opcode  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def mr():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1405_0942_b200 import mr as m
+    return m
+
+
+@pytest.fixture(scope="module", autouse=True)
+def oracle_threads():
+    mro.set_threads(mro.max_threads())
+    yield
+    mro.set_threads(1)
+
+
+# ------------------------------------------------------------------------------------------ S4 exposed: mr_rhs
+
+@pytest.mark.parametrize("name", CASES)
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_rhs_matches_the_oracle_velocity(mr, name, op):
+    """u = gamma J x B (Eq. 1.5) of the RHS instantiation of the step kernels, element by element at 1e-12; exactly 0 on
+    the line-tied boundary nodes."""
+    g, x0, B0, dt = case(name)
+    sim = make_sim(mr, g, x0, B0)
+    u = sim.rhs(op).cpu().numpy()
+    ref = mro.fields(g.n, g.lo, g.hi, x0, B0, op=opcode(op))[2]
+    assert nrel(u, ref) < TOL_STEP
+    m = np.ones(u.shape, bool)
+    m[:, 1:-1, 1:-1, 1:-1] = False
+    assert np.abs(u[m]).max() == 0.0
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), x0) < 1e-15       # the state is untouched
+
+
+def test_displacement_entry_points_round_trip(mr):
+    g, x0, B0, dt = case("ragged")
+    X = I.reference_grid(g)
+    sim = make_sim(mr, g, X, B0)
+    sim.set_xi(dev(x0 - X))
+    assert np.array_equal(sim.get_xi().cpu().numpy(), x0 - X)
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), x0) < 1e-15
+    bad = x0 - X
+    bad[1, 0, 3, 3] = 0.01                                           # a node on a line-tied face off the reference grid
+    with pytest.raises(mr.MrError):
+        sim.set_xi(dev(bad))
+
+
+# ------------------------------------------------------------------------------------------ section 2.4
+
+@pytest.mark.parametrize("name", ["C1", "ragged", "C3_small"])
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+@pytest.mark.parametrize("variant", ["auto", "generic"])
+def test_one_cash_karp_trial_matches_oracle(mr, name, op, variant):
+    """One accepted trial step of a given length: the fifth-order solution within 1e-12, and Lambda = max |x5 - x4|
+    (the oracle forms it from the two solutions, which costs it eps |x| / Lambda ~ 1e-8 of relative accuracy)."""
+    g, x0, B0, dt = case(name)
+    h = 2.0 * dt
+    sim = make_sim(mr, g, x0, B0, variant=variant)
+    st = sim.step_adaptive(t_end=h, lambda0=1e30, dt=h, op=op, trace=True)
+    assert (st["accepted"], st["rejected"], st["rhs_evals"], st["time"]) == (1, 0, 6, h)
+    xr, t, dtn, counts, trace = mro.step_adaptive(g.n, g.lo, g.hi, x0, B0, t_end=h, lam0=1e30, dt=h, op=opcode(op))
+    x = sim.get_fields(x=True)["x"].cpu().numpy()
+    assert nrel(x, xr) < TOL_STEP
+    moved = np.abs(xr - x0).max()
+    assert np.abs(x - xr).max() < 1e-10 * moved + 1e-15 * np.abs(xr).max()
+    assert st["last_lambda"] == pytest.approx(trace[0][2], rel=1e-5, abs=1e-15 * np.abs(xr).max())
+    assert sim.diagnostics(op)["time"] == h
+
+
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_adaptive_run_on_config1_follows_the_oracle(mr, op):
+    """C1 from t = 0 to 0.3 with Lambda0 = 1e-7 and a first trial beyond the stability limit: the same accept / reject
+    sequence as the oracle, the same step lengths, the same end state; the energy decays over the accepted steps."""
+    cfg = I.CONFIGS["C1"]
+    g = cfg.grid
+    x0, B0, _ = I.make(cfg)
+    xr, t, dtn, (acc, rej), trace = mro.step_adaptive(g.n, g.lo, g.hi, x0, B0, t_end=0.3, lam0=1e-7, dt=0.2, op=opcode(op))
+    sim = make_sim(mr, g, x0, B0)
+    st = sim.step_adaptive(t_end=0.3, lambda0=1e-7, dt=0.2, op=op, trace=True)
+    assert (st["accepted"], st["rejected"]) == (acc, rej) and rej >= 1 and st["time"] == 0.3
+    assert [r[3] for r in st["trace"]] == [r[3] for r in trace]
+    for a, b in zip(st["trace"], trace):
+        assert a[0] == pytest.approx(b[0], rel=1e-7, abs=1e-12) and a[1] == pytest.approx(b[1], rel=1e-7)
+        assert a[2] == pytest.approx(b[2], rel=1e-4)
+    assert st["dt_next"] == pytest.approx(dtn, rel=1e-6)
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), xr) < TOL_100
+    # monotone energy over accepted steps (a second context replays them one call at a time)
+    sim2 = make_sim(mr, g, x0, B0)
+    E = [sim2.diagnostics(op)["energy"]]
+    dt = 0.2
+    for target in (0.1, 0.2, 0.3):
+        dt = sim2.step_adaptive(t_end=target, lambda0=1e-7, dt=dt, op=op)["dt_next"]
+        E.append(sim2.diagnostics(op)["energy"])
+    assert all(b < a for a, b in zip(E[:-1], E[1:]))
+
+
+def test_adaptive_needs_state_and_reports_failure(mr):
+    g, x0, B0, dt = case("C1")
+    sim = mr.Relaxation(g.n, g.lo, g.hi)
+    with pytest.raises(mr.MrError) as e:
+        sim.step_adaptive(0.1, 1e-6, 0.01)
+    assert e.value.status == mr.MR_ERR_STATE
+    sim.set_B0(dev(B0))
+    with pytest.raises(mr.MrError) as e:
+        sim.step_adaptive(0.1, -1.0, 0.01)
+    assert e.value.status == mr.MR_ERR_INVALID_ARG
+    with pytest.raises(mr.MrError) as e:                              # two trials cannot reach t_end with dt = 1e-3
+        sim.step_adaptive(0.1, 1e-6, 1e-3, max_trials=2)
+    assert e.value.status == mr.MR_ERR_INVALID_ARG and sim.last_adaptive["accepted"] == 2
+
+
+# ------------------------------------------------------------------------------------------ Eqs. 2.12-2.14
+
+def _periodic_case(bc):
+    n = (20, 12, 10)
+    per = [b == "periodic" for b in bc]
+    lo = (-1.0, -1.0, -1.0)
+    hi = tuple(1.0 - (2.0 / n[a] if per[a] else 0.0) for a in range(3))        # period 2 on a periodic axis
+    g = I.Grid(n, lo, hi)
+    X = I.reference_grid(g)
+    s = [np.pi * (X[a] + 1.0) for a in range(3)]                               # phase 0 .. 2 pi over the period / the box
+    env = np.ones_like(X[0])
+    for a in range(3):
+        if not per[a]:
+            env = env * np.sin(0.5 * s[a])                                     # zero on line-tied faces
+    x = X.copy()
+    x[0] += 0.03 * env * np.sin(s[2] + 0.2) * np.cos(s[1])
+    x[1] += 0.02 * env * np.cos(s[0]) * np.sin(s[2])
+    x[2] += 0.025 * env * np.sin(s[0] + s[1])
+    B0 = np.empty_like(X)
+    B0[0] = 0.3 * np.sin(s[2]) + 0.2 * np.cos(s[1])
+    B0[1] = 0.25 * np.cos(s[0]) * np.sin(s[2])
+    B0[2] = 1.0 + 0.2 * np.sin(s[0]) * np.cos(s[1])
+    return g, x, B0
+
+
+@pytest.mark.parametrize("bc", [("line_tied", "line_tied", "periodic"), ("periodic", "periodic", "periodic"),
+                                ("periodic", "line_tied", "line_tied")])
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_periodic_boundaries_match_oracle(mr, bc, op):
+    g, x0, B0 = _periodic_case(bc)
+    obc = tuple(1 if b == "periodic" else 0 for b in bc)
+    sim = make_sim(mr, g, x0, B0, bc=bc)
+    f = fields_np(sim, op)
+    B, J, u, det = mro.fields(g.n, g.lo, g.hi, x0, B0, op=opcode(op), bc=obc)
+    assert nrel(f["B"], B) < TOL_STEP and nrel(f["J"], J) < TOL_STEP
+    assert nrel(sim.rhs(op).cpu().numpy(), u) < TOL_STEP
+    d, o = sim.diagnostics(op), mro.diagnostics(g.n, g.lo, g.hi, x0, B0, op=opcode(op), bc=obc)
+    for k in ("energy", "max_jxb", "xi", "min_det"):
+        assert d[k] == pytest.approx(o[k], rel=TOL_STEP), k
+    dt = 0.25 * I.stable_dt(B0, g)
+    sim.step(20, dt, op)
+    assert sim.step_variant.startswith("generic")
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 20, op=opcode(op), bc=obc)
+    x = sim.get_fields(x=True)["x"].cpu().numpy()
+    assert nrel(x, ref) < 1e-11
+    pa = [a for a in range(3) if obc[a]][0]                                    # the end plane of a periodic axis moves
+    sl = [slice(None)] * 4
+    sl[3 - pa] = 0
+    assert np.abs(x[tuple(sl)] - x0[tuple(sl)]).max() > 0
+    st = sim.step_adaptive(t_end=sim.diagnostics(op)["time"] + 4 * dt, lambda0=1e-9, dt=dt, op=op)
+    xr, _, _, counts, _ = mro.step_adaptive(g.n, g.lo, g.hi, ref, B0, t_end=4 * dt, lam0=1e-9, dt=dt, op=opcode(op), bc=obc)
+    assert (st["accepted"], st["rejected"]) == counts
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), xr) < 1e-11
+    assert sim.convexity()[0] == mro.convexity(g.n, g.lo, g.hi, xr, bc=obc)[1] == 0
+
+
+# ------------------------------------------------------------------------------------------ Eqs. 3.10-3.11
+
+def test_convexity_matches_oracle(mr):
+    g = I.Grid((37, 21, 13), (-4.0, -4.0, -8.0), (4.0, 4.0, 8.0))
+    B0 = np.zeros(g.shape)
+    B0[2] = 1.0
+    x = I.rough_displacement(g, 0.9, seed=21)                          # 0.9 h random kicks: a good share of concave nodes
+    kap, bad = mro.convexity(g.n, g.lo, g.hi, x)
+    assert 0 < bad < g.nodes
+    sim = make_sim(mr, g, x, B0)
+    n, field = sim.convexity(want_field=True)
+    assert n == bad and np.array_equal(field.cpu().numpy(), kap)
+    assert sim.convexity()[0] == bad
+    sim32 = mr.Relaxation(g.n, g.lo, g.hi, dtype="f32")
+    assert sim32.convexity()[0] == 0                                   # x = X
+
+
+# ------------------------------------------------------------------------------------------ Eqs. 3.5-3.9
+
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_eps_star_and_sigma_match_oracle(mr, op):
+    """IsoHelix (Eq. 3.1) on an odd grid, a few steps in: alpha* along the axis, eps*, sigma_x and sigma_B against the
+    oracle; the references are the exact relaxed state (Eqs. 3.2, 3.3)."""
+    g = I.Grid((17, 17, 21), (-4.0, -4.0, -10.0), (4.0, 4.0, 10.0))
+    phi = np.pi / 4
+    B0 = I.isohelix_B0(g, phi)
+    X = I.reference_grid(g)
+    dt = I.stable_dt(B0, g)
+    sim = make_sim(mr, g, X, B0)
+    sim.step(30, dt, op)
+    x = mro.step(g.n, g.lo, g.hi, X, B0, dt, 30, op=opcode(op))
+    al, eps = sim.eps_star(8, 8, np.sqrt(2.0), op)
+    alr, epsr = mro.eps_star(g.n, g.lo, g.hi, x, B0, 8, 8, np.sqrt(2.0), op=opcode(op))
+    assert np.abs(np.array(al) - alr).max() < 1e-11 * max(np.abs(alr).max(), 1.0)
+    assert eps == pytest.approx(epsr, rel=1e-9) and eps > 0
+    xref = I.isohelix_x_relax(g, phi)
+    Bref = np.zeros(g.shape)
+    Bref[2] = 1.0
+    sx, sb = sim.sigma(dev(xref), dev(Bref))
+    sxr, sbr = mro.sigma(g.n, g.lo, g.hi, x, B0, xref, Bref)
+    assert sx == pytest.approx(sxr, rel=1e-11) and sb == pytest.approx(sbr, rel=1e-11)
+    with pytest.raises(mr.MrError):
+        sim.eps_star(0, 8, 1.0, op)                                    # a line on a line-tied face
+
+
+# ------------------------------------------------------------------------------------------ BASELINE configs[2]
+
+def test_config3_full_size_report_and_parity(mr):
+    """Config 3 at its full 128^3, reading P (B0 pulled back with the ORACLE's Jacobian so that the nodal pushed-forward
+    field is ABC(x0)): fields and both curl errors against the oracle, 100 steps against the oracle, and the field stays
+    near force-free."""
+    cfg = I.CONFIGS["C3"]
+    g = cfg.grid
+    x0 = I.displaced_grid(g, 0.3)
+    F, det = mro.jacobian(g.n, g.lo, g.hi, x0)
+    Fi = np.linalg.inv(np.moveaxis(F, (0, 1), (-2, -1)))
+    B0 = np.ascontiguousarray(np.einsum("...ac,c...->a...", Fi, I.abc_field(x0)) * det)
+    del F, Fi
+    dt = I.stable_dt(B0, g)
+    sim = make_sim(mr, g, x0, B0)
+    errs = {}
+    inner = (slice(None), slice(1, -1), slice(1, -1), slice(1, -1))
+    for op in ("mimetic", "direct"):
+        f = fields_np(sim, op)
+        _, J, _, _ = mro.fields(g.n, g.lo, g.hi, x0, B0, op=opcode(op))
+        assert nrel(f["B"], I.abc_field(x0)) < 1e-12
+        assert nrel(f["J"], J) < TOL_STEP
+        errs[op] = np.abs(f["J"][inner] - np.pi * f["B"][inner]).max() / (np.pi * np.abs(f["B"]).max())
+    assert errs["mimetic"] < errs["direct"] < 2e-3            # second order: (48^3: 7e-3 / 2e-2) x (48/128)^2
+    f0 = sim.diagnostics()["max_jxb"]
+    sim.step(100, dt)
+    d = sim.diagnostics()
+    assert d["max_jxb"] < 2.0 * f0 + 1e-3
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 100)
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), ref) < TOL_100
+    o = mro.diagnostics(g.n, g.lo, g.hi, ref, B0)
+    for k in ("energy", "max_jxb", "min_det"):
+        assert d[k] == pytest.approx(o[k], rel=1e-8), k

@@ -12,9 +12,7 @@ torch = pytest.importorskip("torch")
 from oracle import mro  # noqa: E402  (test infrastructure)
 from paper_1405_0942_b200 import inputs as I  # noqa: E402
 
-TOL_STEP = 1e-12
-TOL_100 = 1e-9
-TOL_F32 = 1e-5
+from gpu_common import CASES, TOL_100, TOL_F32, TOL_STEP, case, dev, fields_np, make_sim, nrel, opcode  # noqa: E402
 
 
 @pytest.fixture(scope="module")
@@ -30,67 +28,6 @@ def oracle_threads():
     mro.set_threads(mro.max_threads())
     yield
     mro.set_threads(1)
-
-
-def nrel(a, b):
-    """norm-wise relative error of a field (Q19)"""
-    return float(np.abs(np.asarray(a) - np.asarray(b)).max() / max(np.abs(b).max(), 1e-300))
-
-
-def dev(a, dtype=torch.float64):
-    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda", dtype=dtype)
-
-
-def make_sim(mr, g, x0, B0, dtype="f64", variant=None):
-    td = torch.float64 if dtype == "f64" else torch.float32
-    sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype)
-    if variant:
-        sim.set_variant(variant)
-    sim.set_B0(dev(B0, td))
-    sim.set_x(dev(x0, td))
-    return sim
-
-
-def fields_np(sim, op):
-    f = sim.get_fields(op, x=True, B=True, J=True)
-    return {k: v.double().cpu().numpy() for k, v in f.items()}
-
-
-def case(name):
-    """(grid, x0, B0, dt) for the parity cases: sizes the oracle finishes in seconds that still span several
-    tiles with a ragged tail."""
-    if name == "C1":
-        cfg = I.CONFIGS["C1"]
-        x0, B0, dt = I.make(cfg)
-        return cfg.grid, x0, B0, dt
-    if name == "C1_rough":      # C1 field on a non-smoothly distorted grid
-        cfg = I.CONFIGS["C1"]
-        _, B0, dt = I.make(cfg)
-        return cfg.grid, I.rough_displacement(cfg.grid, 0.2, seed=5), B0, dt
-    if name == "ragged":        # odd sizes: row padding, partial tiles in every direction
-        g = I.Grid((37, 21, 13), (-4.0, -4.0, -8.0), (4.0, 4.0, 8.0))
-        B0 = I.twist_field(g, (I.Twist(1.0, 0.3, -0.2, 0.4), I.Twist(-0.7, -1.0, 0.5, -3.0)))
-        return g, I.displaced_grid(g, 0.3, seed=7), B0, 0.5 * I.stable_dt(B0, g)
-    if name == "minimal":       # the smallest legal grid
-        g = I.Grid((5, 5, 5), (-1.0, -1.0, -1.0), (1.0, 1.0, 1.0))
-        B0 = I.twist_field(g, (I.Twist(0.5, 0.0, 0.0, 0.0, a=1.0, l=1.0),))
-        return g, I.displaced_grid(g, 0.2, seed=3), B0, 0.25 * I.stable_dt(B0, g)
-    if name == "wide":          # several tiles in x and y, few planes
-        g = I.Grid((130, 70, 9), (-4.0, -4.0, -2.0), (4.0, 4.0, 2.0))
-        B0 = I.twist_field(g, (I.Twist(1.0, 1.0, 0.0, 0.0), I.Twist(-1.0, -1.0, 0.0, 0.5)))
-        return g, I.displaced_grid(g, 0.3, seed=9), B0, 0.5 * I.stable_dt(B0, g)
-    if name == "C2_small":      # config 2 field at a quarter of the resolution
-        cfg = I.scaled(I.CONFIGS["C2"], (32, 32, 96))
-        x0, B0, dt = I.make(cfg)
-        return cfg.grid, x0, B0, dt
-    if name == "C3_small":      # config 3 (reading D) at 48^3
-        cfg = I.scaled(I.CONFIGS["C3"], (48, 48, 48))
-        x0, B0, dt = I.make(cfg)
-        return cfg.grid, x0, B0, dt
-    raise KeyError(name)
-
-
-CASES = ["C1", "C1_rough", "ragged", "minimal", "wide", "C2_small", "C3_small"]
 
 
 @pytest.mark.parametrize("name", CASES)
@@ -124,6 +61,10 @@ def test_one_step_matches_oracle(mr, name, op, variant):
     moved = np.abs(ref - x0).max()
     assert moved > 0
     assert np.abs(x1 - ref).max() < 1e-10 * moved + 1e-15 * np.abs(ref).max()
+    # S4 itself: the velocity of the step kernel's right-hand side against the oracle's u = gamma J x B, at 1e-12
+    u = mro.fields(g.n, g.lo, g.hi, x0, B0, op=opcode(op))[2]
+    sim0 = make_sim(mr, g, x0, B0, variant=variant)
+    assert nrel(sim0.rhs(op).cpu().numpy(), u) < TOL_STEP
     # line-tied: boundary nodes did not move at all
     m = np.ones(x1.shape, bool)
     m[:, 1:-1, 1:-1, 1:-1] = False
@@ -207,9 +148,16 @@ def test_abc_on_undistorted_grid_does_not_move(mr):
     assert sim.diagnostics()["max_jxb"] < 1e-11
 
 
+def rel_dev(a, b):
+    """norm-wise relative difference of two device tensors (Q19), evaluated on the device in fp64"""
+    a, b = a.double(), b.double()
+    return float((a - b).abs().max() / b.abs().max())
+
+
 @pytest.mark.parametrize("variant", ["auto", "generic"])
 def test_fp32_variant_within_1e5_of_fp64(mr, variant):
-    """fp32 storage+arithmetic (displacement storage, Q15) against the fp64 GPU run and the fp64 oracle."""
+    """fp32 storage+arithmetic (displacement storage, Q15) against the fp64 GPU run and the fp64 oracle: every field of
+    north_star's list -- x, B and J -- within 1e-5 norm-wise (Q19), and the displacement itself to 1e-4."""
     cfg = I.scaled(I.CONFIGS["C5"], (64, 64, 64))
     g = cfg.grid
     x0, B0, dt = I.make(cfg)
@@ -217,17 +165,47 @@ def test_fp32_variant_within_1e5_of_fp64(mr, variant):
     s32 = make_sim(mr, g, x0, B0, "f32", variant)
     s64.step(100, dt)
     s32.step(100, dt)
-    x64 = s64.get_fields(x=True)["x"].cpu().numpy()
-    x32 = s32.get_fields(x=True)["x"].double().cpu().numpy()
-    assert nrel(x32, x64) < TOL_F32
-    assert nrel(x32 - x0, x64 - x0) < 1e-3      # even on the displacement itself
+    xi64, xi32 = s64.get_xi(), s32.get_xi()
+    xmax = float(np.abs(x0).max())
+    assert float((xi32.double() - xi64).abs().max()) / xmax < TOL_F32         # x = X + xi, |x| <= 4
+    assert rel_dev(xi32, xi64) < 1e-4                                          # even on the displacement itself
     ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 100)
-    assert nrel(x64, ref) < TOL_100
-    f32, f64 = fields_np(s32, "mimetic"), fields_np(s64, "mimetic")
-    assert nrel(f32["B"], f64["B"]) < TOL_F32
-    assert nrel(f32["J"], f64["J"]) < 1e-3      # J is a difference quotient: eps/h amplification
+    assert nrel(s64.get_fields(x=True)["x"].cpu().numpy(), ref) < TOL_100
+    f32, f64 = s32.get_fields("mimetic", B=True, J=True), s64.get_fields("mimetic", B=True, J=True)
+    assert rel_dev(f32["B"], f64["B"]) < TOL_F32
+    assert rel_dev(f32["J"], f64["J"]) < TOL_F32
     d32, d64 = s32.diagnostics(), s64.diagnostics()
     assert d32["energy"] == pytest.approx(d64["energy"], rel=TOL_F32)
+
+
+def test_fp32_variant_full_size_config5(mr):
+    """BASELINE configs[4] at full size (512^3, the launch configuration bench.py --workload C5 times): the fp32 context
+    against an fp64 context on the same inputs, 100 steps each; x, B and J within 1e-5 norm-wise."""
+    cfg = I.CONFIGS["C5"]
+    g = cfg.grid
+    x0, B0, dt = I.make(cfg)
+    B0t = torch.from_numpy(B0)
+    del x0
+    sims = {}
+    for dtype, td in (("f64", torch.float64), ("f32", torch.float32)):
+        s = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype)
+        s.set_B0(B0t.to("cuda", dtype=td))
+        s.step(100, dt)                                     # starts at x = X: no mr_set_x
+        sims[dtype] = s
+    assert sims["f32"].step_variant == "sym_tmem_f32" and sims["f64"].step_variant == "sym_tmem_f64"
+    xi64, xi32 = sims["f64"].get_xi(), sims["f32"].get_xi()
+    err_x = float((xi32.double() - xi64).abs().max()) / 4.0
+    err_xi = rel_dev(xi32, xi64)
+    del xi64, xi32
+    errs = {"x": err_x, "xi": err_xi}
+    for name in ("B", "J"):
+        a = sims["f32"].get_fields("mimetic", **{name: True})[name]
+        b = sims["f64"].get_fields("mimetic", **{name: True})[name]
+        errs[name] = rel_dev(a, b)
+        del a, b
+    print("fp32 vs fp64 at 512^3 after 100 steps:", errs)
+    assert errs["x"] < TOL_F32 and errs["B"] < TOL_F32 and errs["J"] < TOL_F32, errs
+    assert errs["xi"] < 1e-3, errs
 
 
 def test_host_buffer_entry_points_round_trip(mr):
@@ -304,6 +282,27 @@ def test_full_size_config4_one_step_matches_oracle(mr):
         assert d[k] == pytest.approx(o[k], rel=TOL_STEP), k
 
 
+def test_full_size_config4_direct_operator_matches_oracle(mr):
+    """The direct-derivative operator at the full 256x256x512: one step and the diagnostics (the streaming pass over the
+    inner nodes plus the pass over the faces) against the oracle on the whole grid."""
+    cfg = I.CONFIGS["C4"]
+    g = cfg.grid
+    _, B0, dt = I.make(cfg)
+    x0 = I.displaced_grid(g, 0.3, seed=12)
+    sim = make_sim(mr, g, x0, B0)
+    d = sim.diagnostics("direct")
+    sim.step(1, dt, "direct")
+    assert sim.step_variant == "direct_tma_f64"
+    x1 = sim.get_fields(x=True, host=True)["x"].numpy()
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 1, op=mro.DIRECT)
+    assert nrel(x1, ref) < TOL_STEP
+    moved = np.abs(ref - x0).max()
+    assert np.abs(x1 - ref).max() < 1e-10 * moved + 1e-15 * np.abs(ref).max()
+    o = mro.diagnostics(g.n, g.lo, g.hi, x0, B0, op=mro.DIRECT)
+    for k in ("energy", "max_jxb", "xi", "min_det"):
+        assert d[k] == pytest.approx(o[k], rel=TOL_STEP), k
+
+
 def test_fp32_context_accepts_the_fp32_rounding_of_the_reference_grid(mr):
     """mr_set_x on an fp32 context: boundary nodes given as float32(X) are on the reference grid (|X|/h is large
     on config 5: 4 / (8/511)), one really displaced boundary node is still refused."""
@@ -333,8 +332,7 @@ def test_fp32_direct_operator_within_1e5_of_fp64(mr, variant):
     s32.step(50, dt, "direct")
     assert s64.step_variant == ("direct_tma_f64" if variant == "auto" else "generic_direct")
     x64 = s64.get_fields(x=True)["x"].cpu().numpy()
-    x32 = s32.get_fields(x=True)["x"].double().cpu().numpy()
-    assert nrel(x32, x64) < TOL_F32
+    assert float((s32.get_xi().double() - s64.get_xi()).abs().max()) / float(np.abs(x0).max()) < TOL_F32
     ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 50, op=mro.DIRECT)
     assert nrel(x64, ref) < TOL_100
 
