@@ -1,12 +1,18 @@
 #!/usr/bin/env python
 """bench.py -- grid-point updates/s of the relaxation step (fp64, mimetic curl) on BASELINE.json config 4.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C1..C5]
+                    [--operator mimetic|direct] [--integrator euler|adaptive] [--reading P|D]
 
 One "step" is one pass of the whole hot path (S1-S5: Jacobian, push-forward, mimetic curl, J x B, line-tied
 update) over the full 256x256x512 grid = one fused kernel launch inside mr_step.  The timed region is ONE
 mr_step(K) call bracketed by CUDA events on the launching stream (barrier + synchronize on both sides, max
 over ranks).  Prints ONE JSON line (see DESIGN.md "Measurement" for every key).
+
+Besides the K timed steps the line carries a "burst" record (20 steps at full clocks) and a "sustained" record (a run of at
+least 2 s under the board's power cap, with the clocks it saw): the roofline fraction is quoted for all three.
+--workload C3 adds the report BASELINE configs[2] asks for (both curl errors at t = 0, max |J x B| and |x - x0| after the
+steps); --integrator adaptive times the Cash-Karp integrator of section 2.4 in right-hand-side evaluations per second.
 
 Multi-GPU: north_star keeps the path on one GPU ("replicas only"): --gpus N runs N independent
 replicas, one process per GPU (torchrun), value = N * nodes * K / max-over-ranks time, "scaling": "weak".
@@ -50,14 +56,27 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def csrc_fingerprint():
+    """sha1 over the CUDA sources: a traffic row is only valid for the sources it was captured with."""
+    import glob
+    import hashlib
+    h = hashlib.sha1()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1405_0942_b200", "csrc", "*"))):
+        with open(f, "rb") as fh:
+            h.update(os.path.basename(f).encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
 def recorded_traffic(workload, kernel):
-    """dram bytes per launch of this step kernel from the committed ncu --set full capture (profiles/traffic.csv,
-    written by hand from the summary it names), or None if this variant has not been captured."""
+    """dram bytes per launch of this step kernel from the committed ncu --set full capture (profiles/traffic.csv, one row
+    per capture with the fingerprint of the sources it was taken with), or None if there is no capture of THESE sources:
+    a stale row is never printed."""
     import csv
     try:
+        fp = csrc_fingerprint()
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == workload and row["kernel"] == kernel:
+                if row["workload"] == workload and row["kernel"] == kernel and row.get("csrc_sha1") == fp:
                     return float(row["dram_bytes_per_launch"])
     except Exception:
         pass
@@ -176,7 +195,7 @@ def run_reference(args):
     g = cfg.grid
     planes = 16
     sub = I.Grid((g.n[0], g.n[1], planes), g.lo, (g.hi[0], g.hi[1], g.lo[2] + (planes - 1) * g.h[2]))
-    B0 = I.twist_field(sub, cfg.twists)
+    B0 = I.twist_field(sub, cfg.twists) if cfg.twists else I.abc_field(I.reference_grid(sub))
     x = I.reference_grid(sub)
     dt = I.stable_dt(B0, sub)
     threads = mro.max_threads()
@@ -204,13 +223,31 @@ def run_reference(args):
 
 # ---------------------------------------------------------------------------------------------- our arm (GPU)
 
+def reading_P_field(I, g, x0):
+    """Config 3, reading P (Q16): B(X,0) pulled back so that the nodal pushed-forward field equals ABC(x0).  The
+    discrete Jacobian is numpy.gradient's (second-order central inside, second-order one-sided on the faces: the same
+    stencil as reading Q3), so neither the product nor the oracle is involved in making the input."""
+    import numpy as np
+    F = np.empty((3, 3) + x0.shape[1:])
+    for c in range(3):
+        for a in range(3):
+            F[c, a] = np.gradient(x0[c], g.h[a], axis=2 - a, edge_order=2)
+    Fm = np.moveaxis(F, (0, 1), (-2, -1))
+    det = np.linalg.det(Fm)
+    Fi = np.linalg.inv(Fm)
+    return np.ascontiguousarray(np.einsum("...ac,c...->a...", Fi, I.abc_field(x0)) * det)
+
+
 def run_ours(args):
+    import numpy as np
     import torch
     import torch.distributed as dist
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d: launch N ranks with torch.distributed.run (one per GPU)" % (args.gpus, world))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the relaxation step has no CPU path")
     torch.cuda.set_device(local_rank)
@@ -223,52 +260,126 @@ def run_ours(args):
     dtype = cfg.dtype
     td = torch.float64 if dtype == "f64" else torch.float32
     x0, B0, dt = I.make(cfg)
+    if cfg.kind == "abc" and args.reading == "P":
+        B0 = reading_P_field(I, g, x0)
+        dt = I.stable_dt(B0, g)
     nodes = g.nodes
+    X = I.reference_grid(g)
+    displaced = not np.array_equal(x0, X)
 
     sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype, device="cuda:%d" % local_rank)
     if args.variant != "auto":
         sim.set_variant(args.variant)
-    B0_d = torch.from_numpy(B0).to("cuda", dtype=td)
-    x0_d = torch.from_numpy(x0).to("cuda", dtype=td)
-    sim.set_B0(B0_d)
-    sim.set_x(x0_d)
-    del B0_d
+    sim.set_B0(torch.from_numpy(B0).to("cuda", dtype=td))
+
+    def reset_state():
+        """back to the initial state: an fp32 context takes the displacement (Q15); x = X needs the zero displacement"""
+        if dtype == "f64":
+            sim.set_x(torch.from_numpy(x0).to("cuda", dtype=td))
+        else:
+            sim.set_xi(torch.from_numpy(x0 - X).to("cuda", dtype=td))
+
+    if displaced:
+        reset_state()                                  # (a context starts at x = X: nothing to set otherwise)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident throughput: W warm-up steps, then ONE timed mr_step(K) ----
     op = args.operator
-    sim.step(max(args.warmup, 3), dt, op)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    with ClockSampler(local_rank) as clocks:
-        l0 = sim.launch_count
-        e0.record()
-        sim.step(args.steps, dt, op)
-        e1.record()
-        barrier()
-        launches = sim.launch_count - l0
-    ms = e0.elapsed_time(e1)
-    variant = sim.step_variant
-    ms_all, updates_all = aggregate_over_ranks(ms, nodes * args.steps, dist if world > 1 else None)
-    value = updates_all / (ms_all * 1e-3)
-    diag = sim.diagnostics(op)
+    report = None
+    if cfg.kind == "abc":
+        # BASELINE configs[2]: "the mimetic and direct curl errors are reported" (exact curl of an ABC field: pi B)
+        report = {"reading": args.reading, "dt": dt}
+        inner = (slice(None), slice(1, -1), slice(1, -1), slice(1, -1))
+        for o in ("mimetic", "direct"):
+            f = sim.get_fields(o, B=True, J=True)
+            Bf, Jf = f["B"][inner], f["J"][inner]
+            report["curl_error_" + o] = float((Jf - np.pi * Bf).abs().max() / (np.pi * f["B"].abs().max()))
+            del f, Bf, Jf
+        d0 = sim.diagnostics(op)
+        report.update({"max_jxb_0": d0["max_jxb"], "xi_0": d0["xi"], "energy_0": d0["energy"]})
+        sim.step(cfg.steps, dt, op)                    # the config's 200 steps, then back to the initial state for the timing
+        d1 = sim.diagnostics(op)
+        xi_0 = torch.from_numpy(x0 - X).to("cuda")
+        report.update({"steps": cfg.steps, "max_jxb_after": d1["max_jxb"], "xi_after": d1["xi"], "energy_after": d1["energy"],
+                       "max_abs_x_minus_x0": float((sim.get_xi().double() - xi_0).abs().max()), "h": g.h[0],
+                       "concave_nodes_after": sim.convexity()[0]})
+        del xi_0
+        reset_state()
 
-    # ---- roofline of the dominant (only) kernel: algorithmic bytes per launch / average launch duration ----
+    def timed(steps):
+        """CUDA events around ONE mr_step(steps) (or one mr_step_adaptive of `steps` trial steps' worth of time)"""
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        with ClockSampler(local_rank) as clocks:
+            l0 = sim.launch_count
+            e0.record()
+            sim.step(steps, dt, op)
+            e1.record()
+            barrier()
+            launches = sim.launch_count - l0
+        ms = e0.elapsed_time(e1)
+        ms_all, updates_all = aggregate_over_ranks(ms, nodes * steps, dist if world > 1 else None)
+        return {"ms": ms, "ms_all": ms_all, "updates_all": updates_all, "launches": launches, "clocks": clocks.summary(), "steps": steps}
+
+    # ---- device-resident throughput: W warm-up steps, then ONE timed mr_step(K) ----
+    W = max(args.warmup, 3)
+    sim.step(W, dt, op)
+    main = timed(args.steps)
+    variant = sim.step_variant
+    value = main["updates_all"] / (main["ms_all"] * 1e-3)
+    diag = sim.diagnostics(op)
     peak, peak_src = measured_peak_gbs()
-    launch_ms = ms / max(launches, 1)
-    achieved = BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+
+    def roof(rec):
+        launch_ms = rec["ms"] / max(rec["launches"], 1)
+        if op == "direct":
+            tf = DIRECT_FLOP_PER_UPDATE * nodes / (launch_ms * 1e-3) / 1e12
+            return {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
+                    "traffic": None, "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 x 1.965 GHz", "kernel": variant,
+                    "algorithmic_flop_per_launch": DIRECT_FLOP_PER_UPDATE * nodes, "launch_ms": launch_ms,
+                    "hbm_frac": BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9 / peak}
+        achieved = BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9
+        return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": recorded_traffic(cfg.name, variant), "peak_source": peak_src, "kernel": variant,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE[dtype] * nodes, "launch_ms": launch_ms}
-    if op == "direct":
-        tf = DIRECT_FLOP_PER_UPDATE * nodes / (launch_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
-                    "traffic": None, "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 x 1.965 GHz", "kernel": variant,
-                    "algorithmic_flop_per_launch": DIRECT_FLOP_PER_UPDATE * nodes, "launch_ms": launch_ms}
+
+    roofline = roof(main)
+
+    # ---- the two regimes of this board (1 kW cap): a 20-step burst at full clocks and a run of >= 2 s under the cap ----
+    regimes = {}
+    fbytes = 3 * nodes * (8 if dtype == "f64" else 4)
+    if not args.no_regimes and 3 * fbytes > 4e8:       # (L2-resident workloads: the HBM fraction is n/a, and a long run of a
+                                                       # small braid ends where the paper says it does, PAPER.md:333)
+        ms_step = main["ms"] / args.steps
+        for name, steps in (("burst", 20), ("sustained", int(max(200, min(200000, 2200.0 / max(ms_step, 1e-3)))))):
+            if name == "burst":
+                time.sleep(1.0)                       # let the board cool off the previous run
+            r = timed(steps)
+            rf = roof(r)
+            regimes[name] = {"steps": steps, "ms_per_step": r["ms_all"] / steps, "seconds": r["ms"] * 1e-3,
+                             "value": r["updates_all"] / (r["ms_all"] * 1e-3), "roofline_frac": rf["frac"], "clocks": r["clocks"]}
+
+    # ---- section 2.4: the adaptive Cash-Karp integrator, in right-hand-side evaluations per second ----
+    adaptive = None
+    if args.integrator == "adaptive":
+        reset_state()
+        lam0 = args.lambda0
+        st = sim.step_adaptive(t_end=3.0 * dt, lambda0=lam0, dt=dt, op=op)         # warm-up (binds the workspace)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        t0 = sim.diagnostics(op)["time"]
+        e0.record()
+        st = sim.step_adaptive(t_end=t0 + args.adaptive_span * dt, lambda0=lam0, dt=st["dt_next"], op=op, max_trials=args.steps)  \
+            if args.adaptive_span > 0 else st
+        e1.record()
+        barrier()
+        ams = e0.elapsed_time(e1)
+        adaptive = {"lambda0": lam0, "accepted": st["accepted"], "rejected": st["rejected"], "rhs_evals": st["rhs_evals"],
+                    "ms": ams, "rhs_evals_per_s": st["rhs_evals"] / (ams * 1e-3), "node_rhs_per_s": st["rhs_evals"] * nodes / (ams * 1e-3),
+                    "time_advanced": st["time"] - t0, "dt_next": st["dt_next"], "euler_dt": dt}
 
     # ---- end to end through the host-buffer entry points: H2D of x, one step, D2H of x, every step ----
     xh = torch.from_numpy(x0).to(td).pin_memory()
@@ -287,7 +398,6 @@ def run_ours(args):
     barrier()
     e2e_ms = (time.perf_counter() - t0) * 1e3
     e2e_ms_all, e2e_updates = aggregate_over_ranks(e2e_ms, nodes * e2e_steps, dist if world > 1 else None)
-    fbytes = 3 * nodes * (8 if dtype == "f64" else 4)
     e2e = {"value": e2e_updates / (e2e_ms_all * 1e-3), "unit": UNIT, "h2d_bytes_per_step": fbytes,
            "d2h_bytes_per_step": fbytes, "steps": e2e_steps,
            "what": "per step: mr_set_x_host (pinned H2D of x) + mr_step(1) + mr_get_fields_host (D2H of x)"}
@@ -298,18 +408,24 @@ def run_ours(args):
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
 
     if rank == 0:
+        prec = "fp64" if dtype == "f64" else "fp32"
         line = {
-            "metric": (METRIC if op == "mimetic" else METRIC.replace("mimetic", "direct")).replace("fp64", "fp64" if dtype == "f64" else "fp32"), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": dtype, "data": "synthetic",
-            "config": {"workload": "%s %dx%dx%d %s %s, line-tied, forward Euler dt=%.3e" % ((cfg.name,) + g.n + ("fp64" if dtype == "f64" else "fp32", op, dt)),
-                       "nodes": nodes, "l2_policy": "working set %.2f GB >> 126 MB L2 (no flush needed)" % (3 * fbytes / 1e9),
+            "metric": METRIC.replace("mimetic", op).replace("fp64", prec), "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": W, "ms_per_step": main["ms_all"] / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+            "config": {"workload": "%s %dx%dx%d %s %s, line-tied, forward Euler dt=%.3e" % ((cfg.name,) + g.n + (prec, op, dt)),
+                       "nodes": nodes, "l2_policy": "working set %.2f GB vs 126 MB L2%s" % (3 * fbytes / 1e9, " (no flush needed)" if 3 * fbytes > 4e8 else " (L2-resident: HBM fraction n/a)"),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "kernel": variant},
-            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "clocks": main["clocks"], "e2e": e2e, "gpu_launches": main["launches"], "roofline": roofline,
+            "burst": regimes.get("burst"), "sustained": regimes.get("sustained"),
             "cpu_baseline": cpu_baseline,
             "state_after": {"steps": diag["steps"], "energy": diag["energy"], "max_jxb": diag["max_jxb"], "xi": diag["xi"],
                             "min_det": diag["min_det"]},
         }
+        if report is not None:
+            line["config3_report"] = report
+        if adaptive is not None:
+            line["adaptive"] = adaptive
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -322,11 +438,16 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C4", "C5"])
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--variant", default="auto", choices=["auto", "generic"])
     ap.add_argument("--operator", default="mimetic", choices=["mimetic", "direct"])
+    ap.add_argument("--integrator", default="euler", choices=["euler", "adaptive"])
+    ap.add_argument("--reading", default="P", choices=["P", "D"], help="config 3: B0 pulled back (P) or ABC(X) literally (D)")
+    ap.add_argument("--lambda0", type=float, default=1e-9, help="tolerance of the adaptive integrator")
+    ap.add_argument("--adaptive-span", type=float, default=40.0, help="time to advance in the adaptive run, in Euler steps dt")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-regimes", action="store_true", help="skip the burst / sustained records")
     args = ap.parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)

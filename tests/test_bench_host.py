@@ -57,8 +57,31 @@ def test_roofline_denominator_and_bytes_per_update():
     peak, src = bench.measured_peak_gbs()
     assert peak > 1000.0 and ("measured" in src or "fallback" in src)
     assert bench.BYTES_PER_UPDATE == {"f64": 72.0, "f32": 36.0}      # read xi + read b + write xi', 3 components each
-    t = bench.recorded_traffic("C4", "duo_tmem_f64")
+    t = bench.recorded_traffic("C4", "sym_tmem_f64")
     assert t is None or 0.9 < t / (72.0 * 256 * 256 * 512) < 1.5
+
+
+def test_traffic_rows_of_other_sources_are_never_printed(tmp_path, monkeypatch):
+    """roofline.traffic comes from a committed ncu capture; a row taken with other CUDA sources must not be quoted."""
+    fp = bench.csrc_fingerprint()
+    assert len(fp) == 16 and fp == bench.csrc_fingerprint()
+    prof = tmp_path / "profiles"
+    prof.mkdir()
+    (prof / "traffic.csv").write_text("workload,kernel,dram_bytes_per_launch,csrc_sha1,source\n"
+                                      "C4,sym_tmem_f64,2400000000,0123456789abcdef,stale\n"
+                                      "C4,direct_tma_f64,2410000000,%s,fresh\n" % fp)
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))
+    monkeypatch.setattr(bench, "csrc_fingerprint", lambda: fp)
+    assert bench.recorded_traffic("C4", "sym_tmem_f64") is None
+    assert bench.recorded_traffic("C4", "direct_tma_f64") == 2410000000.0
+
+
+def test_gpus_flag_must_match_the_launch():
+    """--gpus N without N launched ranks must fail instead of printing n_gpus: 1 (run plain, WORLD_SIZE is 1)."""
+    env = dict(os.environ, WORLD_SIZE="1")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "8", "--steps", "1"], capture_output=True, text=True,
+                         timeout=300, cwd=ROOT, env=env)
+    assert out.returncode != 0 and "WORLD_SIZE" in (out.stderr + out.stdout)
 
 
 def test_reference_arm_prints_one_json_line_on_cpu():
