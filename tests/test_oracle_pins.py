@@ -280,7 +280,7 @@ def test_direct_equals_mimetic_on_undistorted_grid():
 def test_direct_exact_for_quadratic_map_and_field_sympy():
     """Quadratic map and quadratic B0: all differences in O4d are exact, so J equals the analytic curl of
     F B0 / Delta (computed symbolically with sympy).  The mimetic operator is only O(h^2) here."""
-    sp = pytest.importorskip("sympy")
+    import sympy as sp          # a hard requirement: without it O4d would silently lose its only analytic pin
     g = grid((7, 8, 9), (-1, -1, -1), (1, 1.5, 2))
     x, _, (lin, quad) = quad_map(g, amp=0.05, seed=43)
     rng = np.random.default_rng(44)
