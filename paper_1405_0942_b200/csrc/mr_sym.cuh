@@ -26,6 +26,7 @@
 #include <type_traits>
 
 #include "mr_generic.cuh"
+#include "mr_lanes.cuh"
 #include "mr_stream_common.cuh"
 #include "mr_tmem.cuh"
 
@@ -33,8 +34,9 @@ namespace mr {
 
 template <typename T>
 struct SymLayout {
-    static constexpr int TX = 32, TY = 16, R = 4, NB = 4;
-    static constexpr int HXL = 16 / (int)sizeof(T), HXR = 2 * HXL;
+    static constexpr int NV = Lanes<T>::NV;                         // nodes per thread along i (fp64: 1, fp32: 2)
+    static constexpr int TX = 32 * NV, TY = 16, R = 4, NB = 4;
+    static constexpr int HXL = 16 / (int)sizeof(T), HXR = 2 * HXL;  // x halo: 16 / 32 bytes (TMA alignment), >= NV + 1 nodes
     static constexpr int BW = TX + HXL + HXR;
     static constexpr int XH = TY + 4, BH = TY + 2;
     static constexpr int CSX = BW * XH, CSB = BW * BH;
@@ -42,7 +44,7 @@ struct SymLayout {
     static constexpr int SLOTX = round128(3 * CSX * (int)sizeof(T)) / (int)sizeof(T);
     static constexpr int SLOTB = round128(3 * CSB * (int)sizeof(T)) / (int)sizeof(T);
     static constexpr uint32_t XBOX_BYTES = 3u * CSX * sizeof(T), BBOX_BYTES = 3u * CSB * sizeof(T);
-    static constexpr int BBW = TX + 2, BBH = TY + 2;
+    static constexpr int BBW = TX + 2 * NV, BBH = TY + 2;           // B plane: the tile and one (aligned) thread column either side
     static constexpr int BCS = BBW * BBH;
     static constexpr int BSLOT = round128(3 * BCS * (int)sizeof(T)) / (int)sizeof(T);
     static constexpr int NTW = TY, NWARPS = TY + 4, NTHREADS = NWARPS * 32;     // tile warps + 4 ring warps
@@ -52,7 +54,7 @@ struct SymLayout {
     static constexpr size_t OFF_BAR = OFF_BB + (size_t)NB * BSLOT * sizeof(T);
     static constexpr size_t BYTES = OFF_BAR + (size_t)NB * 8 + 128;
     // TMEM record of a node: chunk 0 = columns 0, 1 of dF, n_0[0], n_0[1] (8 values), chunk 1 = column 2 of dF, n_0[2]
-    static constexpr int WN = (int)sizeof(T) / 4;                   // 32-bit words per value
+    static constexpr int WN = (int)sizeof(typename Lanes<T>::V) / 4;     // 32-bit words per value (a double or a pair of floats)
     #ifdef MR_X_TMEM
     static constexpr int C0W = 8 * WN, C1W = 8 * WN, REC = 16 * WN; // + own xi (3 values) in chunk 1
 #else
@@ -63,6 +65,15 @@ struct SymLayout {
 
 template <int Q> using Phase = std::integral_constant<int, Q>;
 
+namespace tmem {
+template <> struct Words<f2> {
+    static constexpr int N = 2;
+    static __device__ __forceinline__ void put(uint32_t* w, f2 v) { w[0] = __float_as_uint(v.x); w[1] = __float_as_uint(v.y); }
+    static __device__ __forceinline__ f2 get(const uint32_t* w) { return f2{ __uint_as_float(w[0]), __uint_as_float(w[1]) }; }
+};
+}  // namespace tmem
+inline __device__ double Lanes<double>::rcp(double d) { return fast_rcp(d); }
+
 enum : int { MODE_STEP = 0, MODE_DIAG = 1, MODE_RHS = 2 };     // xi+ = xi + dt u  |  the reduction S6  |  out = u = gamma J x B
 
 template <typename T, int MODE>
@@ -71,8 +82,11 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
            T* __restrict__ out, const StreamArgs<T> a)
 {
     using L = SymLayout<T>;
-    using W32 = tmem::Words<T>;
+    using LN = Lanes<T>;
+    using V = typename LN::V;                      // what a thread owns along i: one double, or a packed pair of floats
+    using W32 = tmem::Words<V>;
     constexpr bool DIAG = MODE == MODE_DIAG, RHS = MODE == MODE_RHS;
+    constexpr int NV = L::NV;
     constexpr int TX = L::TX, TY = L::TY, NTW = L::NTW, BW = L::BW, CSX = L::CSX, CSB = L::CSB, BBW = L::BBW, BCS = L::BCS;
     constexpr int NW = L::NWARPS, WN = L::WN, C0W = L::C0W, C1W = L::C1W, REC = L::REC;
     static_assert(L::TMEM_COLS == 256 || L::TMEM_COLS == 128, "TMEM columns: a power of two");
@@ -95,7 +109,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int kend = min(k1, nz - 1);               // planes k0 .. kend-1 are finished here (and nz-1 carried through)
     const int first_p = max(k0 - 1, 0);             // B is formed on the planes first_p .. kend
     const int plast = min(kend + 1, nz - 1);        // last xi / b plane this item touches
-    const T twoh[3] = { a.twoh[0], a.twoh[1], a.twoh[2] };
+    const V twoh[3] = { LN::bc(a.twoh[0]), LN::bc(a.twoh[1]), LN::bc(a.twoh[2]) };
 
     const bool pwarp = warp == NW - 1, producer = pwarp && lane == 0;
     if (producer) {
@@ -140,55 +154,87 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     // row above, both columns) or none (the producer's warp)
     int ti, tj;
     bool has_node = true;
-    if (tilew) { ti = lane; tj = warp; }
-    else if (warp == NTW) { ti = lane; tj = -1; }
-    else if (warp == NTW + 1) { ti = lane; tj = TY; }
-    else if (warp == NTW + 2) { ti = (lane >> 3) & 1 ? TX : -1; tj = (lane & 7) + 8 * (lane >> 4); }
+    if (tilew) { ti = NV * lane; tj = warp; }
+    else if (warp == NTW) { ti = NV * lane; tj = -1; }
+    else if (warp == NTW + 1) { ti = NV * lane; tj = TY; }
+    else if (warp == NTW + 2) { ti = (lane >> 3) & 1 ? TX : -NV; tj = (lane & 7) + 8 * (lane >> 4); }
     else { ti = 0; tj = 0; has_node = false; }
-    const int gi = i0 + ti, gj = j0 + tj;
-    const T* px = sx + (tj + 2) * BW + (ti + L::HXL);       // this node in component 0 of the ring position 0 (xi, b, B)
+    const int gi = i0 + ti, gj = j0 + tj;                   // (first) node of this thread; the second one is gi + 1
+    const T* px = sx + (tj + 2) * BW + (ti + L::HXL);       // this thread in component 0 of the ring position 0 (xi, b, B)
     const T* pb = sb + (tj + 1) * BW + (ti + L::HXL);
-    T* pB = sB + (tj + 1) * BBW + (ti + 1);
-    const bool dom = has_node && gi >= 0 && gi < a.nx && gj >= 0 && gj < a.ny;
-    const unsigned edge = !dom ? 0u : (gi == 0 ? 1u : 0u) | (gi == a.nx - 1 ? 2u : 0u) | (gj == 0 ? 4u : 0u) | (gj == a.ny - 1 ? 8u : 0u);
-    const bool in_xy = gi > 0 && gi < a.nx - 1 && gj > 0 && gj < a.ny - 1;
-    const bool st = tilew && dom;
+    T* pB = sB + (tj + 1) * BBW + (ti + NV);
+    // per node e of the thread: inside the grid / on which faces (1: i = 0, 2: i = nx-1, 4: j = 0, 8: j = ny-1) / interior in xy
+    bool dom[NV], in_xy[NV], st[NV];
+    unsigned edge = 0u;                                     // bits of the node e shifted by 8 e (bits 16, 32 of `special`: the k faces)
+    bool any_st = false;
+    const bool row_in = gj >= 0 && gj < a.ny;
+#pragma unroll
+    for (int e = 0; e < NV; ++e) {
+        const int g = gi + e;
+        dom[e] = has_node && row_in && g >= 0 && g < a.nx;
+        in_xy[e] = g > 0 && g < a.nx - 1 && gj > 0 && gj < a.ny - 1;
+        st[e] = tilew && dom[e];
+        any_st = any_st || st[e];
+        if (dom[e]) edge |= ((g == 0 ? 1u : 0u) | (g == a.nx - 1 ? 2u : 0u) | (gj == 0 ? 4u : 0u) | (gj == a.ny - 1 ? 8u : 0u)) << (8 * e);
+    }
 
     bool ok = true;
-    T xh[2][3], Bh[4][3], sh[2];                             // own xi(p), xi(p-1); own B(p) .. B(p-3); dt gamma / D of p, p-1
+    V xh[2][3], Bh[4][3], sh[2];                             // own xi(p), xi(p-1); own B(p) .. B(p-3); dt gamma / D of p, p-1
+    // a value of this thread's node(s) straight from global memory (0 outside the grid)
+    auto from_global = [&](const T* f, long long o) {
+        V v = LN::bc(T(0));
+#pragma unroll
+        for (int e = 0; e < NV; ++e)
+            if (dom[e]) LN::set(v, e, f[o + e]);
+        return v;
+    };
     {
         // own xi of the plane below the first one (for the first k-difference) straight from global memory
         const long long o = (long long)(first_p - 1) * a.plane + (long long)gj * a.pitch + gi;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            xh[0][c] = T(0);
-            xh[1][c] = (first_p > 0 && dom) ? in[c * a.comp + o] : T(0);        // phase 0 reads xi(first_p - 1) from xh[1]
+            xh[0][c] = LN::bc(T(0));
+            xh[1][c] = first_p > 0 ? from_global(in + c * a.comp, o) : LN::bc(T(0));     // phase 0 reads xi(first_p - 1) from xh[1]
 #pragma unroll
-            for (int q = 0; q < 4; ++q) Bh[q][c] = T(0);
+            for (int q = 0; q < 4; ++q) Bh[q][c] = LN::bc(T(0));
         }
     }
-    sh[0] = sh[1] = T(0);
-#ifndef MR_BM_REG
+    sh[0] = sh[1] = LN::bc(T(0));
     if (tilew) {         // the first F reads the own B of the plane first_p - 1 (never formed) from the B plane 3: a finite stand-in
 #pragma unroll
-        for (int c = 0; c < 3; ++c) pB[3 * L::BSLOT + c * BCS] = T(0);
+        for (int c = 0; c < 3; ++c) LN::st(pB + 3 * L::BSLOT + c * BCS, LN::bc(T(0)));
     }
-#endif
     T* po = out + (long long)first_p * a.plane + (long long)gj * a.pitch + gi;     // plane t = p-1 of the first F
+    // store the thread's node(s) that lie inside the grid
+    auto store_nodes = [&](T* q, V v) {
+        if (NV == 2 && st[0] && st[NV - 1]) { LN::st(q, v); return; }
+#pragma unroll
+        for (int e = 0; e < NV; ++e)
+            if (st[e]) q[e] = LN::get(v, e);
+    };
     DiagPartial acc = { 0.0, 0.0, 0.0, INFINITY };          // DIAG: this thread's partial
-    const double zxy = ((gi == 0 || gi == a.nx - 1) ? 0.5 : 1.0) * ((gj == 0 || gj == a.ny - 1) ? 0.5 : 1.0);   // Eq. 3.13
-    auto diag_node = [&](int k, const T(&c0)[3], const T(&n0)[3], const T(&B)[3], const T(&uu)[3]) {
-        if (!st) return;
-        const double D = (double)c0[0] * n0[0] + (double)c0[1] * n0[1] + (double)c0[2] * n0[2];
-        const double b2 = (double)B[0] * B[0] + (double)B[1] * B[1] + (double)B[2] * B[2];
-        const bool kface = k == 0 || k == nz - 1;
-        DiagPartial v = { zxy * (kface ? 0.5 : 1.0) * b2 * D, 0.0, 0.0, D };
-        if (in_xy && !kface) {
-            const double fm = sqrt((double)uu[0] * uu[0] + (double)uu[1] * uu[1] + (double)uu[2] * uu[2]) / D;
-            v.fmax = fm;
-            v.xi = fm / b2;
+    auto diag_node = [&](int k, const V(&c0)[3], const V(&n0)[3], const V(&B)[3], const V(&uu)[3]) {
+#pragma unroll
+        for (int e = 0; e < NV; ++e) {
+            if (!st[e]) continue;
+            const int g = gi + e;
+            const double zxy = ((g == 0 || g == a.nx - 1) ? 0.5 : 1.0) * ((gj == 0 || gj == a.ny - 1) ? 0.5 : 1.0);   // Eq. 3.13
+            double D = 0.0, b2 = 0.0, u2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                D += (double)LN::get(c0[c], e) * (double)LN::get(n0[c], e);
+                b2 += (double)LN::get(B[c], e) * (double)LN::get(B[c], e);
+                u2 += (double)LN::get(uu[c], e) * (double)LN::get(uu[c], e);
+            }
+            const bool kface = k == 0 || k == nz - 1;
+            DiagPartial v = { zxy * (kface ? 0.5 : 1.0) * b2 * D, 0.0, 0.0, D };
+            if (in_xy[e] && !kface) {
+                const double fm = sqrt(u2) / D;
+                v.fmax = fm;
+                v.xi = fm / b2;
+            }
+            diag_combine(acc, v);
         }
-        diag_combine(acc, v);
     };
 
     if (!pwarp) {        // the planes first_p, first_p + 1 and, for the one-sided difference on the bottom face, 2
@@ -196,9 +242,6 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         ptx::mbar_wait(bar + 16u, 0u);
         if (first_p == 0) ptx::mbar_wait(bar + 24u, 0u);
     }
-#ifdef MR_STAGGER
-    if (tilew && (warp & 1)) __nanosleep(MR_STAGGER);
-#endif
     int p = first_p;
     uint32_t gpar = 0u;                                      // parity of the group of four planes
     auto body = [&](auto phase, auto tile_c) {
@@ -206,59 +249,76 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         constexpr bool TILE = decltype(tile_c)::value;
         constexpr int S0 = (Q + 1) & 3, S1 = (Q + 2) & 3, S2 = (Q + 3) & 3;      // ring positions of the planes p, p+1, p+2 (= p-2)
         constexpr int QM1 = (Q + 3) & 3, QM2 = (Q + 2) & 3;                      // B planes / own B of p-1, p-2
-        T(&x1)[3] = xh[Q & 1];
-        const T(&xp)[3] = xh[(Q + 1) & 1];
-        T(&Bp)[3] = Bh[Q];
+        V(&x1)[3] = xh[Q & 1];
+        const V(&xp)[3] = xh[(Q + 1) & 1];
+        V(&Bp)[3] = Bh[Q];
         const bool fin = TILE && p > first_p;
-        // ---------------- A(p): push-forward of the plane p at the own node ----------------
+        // ---------------- A(p): push-forward of the plane p at the own node(s) ----------------
         const bool work = TILE || (has_node && p < kend);
         const T* fr = px + S0 * L::SLOTX;
         if (work) {
-            const T* f2 = px + S1 * L::SLOTX;
-            T dF[3][3], bq[3];
+            const T* f2p = px + S1 * L::SLOTX;
+            V dF[3][3], bq[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                x1[c] = fr[c * CSX];
-                dF[c][0] = fr[c * CSX + 1] - fr[c * CSX - 1];
-                dF[c][1] = fr[c * CSX + BW] - fr[c * CSX - BW];
-                dF[c][2] = f2[c * CSX] - xp[c];
-                bq[c] = pb[S0 * L::SLOTB + c * CSB];
+                x1[c] = LN::ld(fr + c * CSX);
+                dF[c][0] = LN::di(fr + c * CSX, x1[c]);
+                dF[c][1] = LN::ld(fr + c * CSX + BW) - LN::ld(fr + c * CSX - BW);
+                dF[c][2] = LN::ld(f2p + c * CSX) - xp[c];
+                bq[c] = LN::ld(pb + S0 * L::SLOTB + c * CSB);
             }
             const unsigned special = edge | (p == 0 ? 16u : 0u) | (p == nz - 1 ? 32u : 0u);
             if (special) {
                 if (special & 16u) {            // bottom face: -3 x(0) + 4 x(1) - x(2)
                     const T* f3 = px + S2 * L::SLOTX;
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) dF[c][2] = T(4) * f2[c * CSX] - T(3) * x1[c] - f3[c * CSX];
+                    for (int c = 0; c < 3; ++c) dF[c][2] = LN::bc(T(4)) * LN::ld(f2p + c * CSX) - LN::bc(T(3)) * x1[c] - LN::ld(f3 + c * CSX);
                 }
                 if (special & 32u) {            // top face: 3 x(nz-1) - 4 x(nz-2) + x(nz-3); the own xi of the plane nz-3 comes from
                                                 // global memory (once per column; a last chunk of one plane never loads that plane)
                     const long long o3 = (long long)(nz - 3) * a.plane + (long long)gj * a.pitch + gi;
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) dF[c][2] = T(3) * x1[c] - T(4) * xp[c] + (dom ? in[c * a.comp + o3] : T(0));
+                    for (int c = 0; c < 3; ++c) dF[c][2] = LN::bc(T(3)) * x1[c] - LN::bc(T(4)) * xp[c] + from_global(in + c * a.comp, o3);
                 }
-                if (special & 15u) face_fix<T, BW, CSX>(fr, special & 15u, dF);
+                // one-sided in-plane differences of a node on an x / y face (reading Q3), node by node
+#pragma unroll
+                for (int e = 0; e < NV; ++e) {
+                    const unsigned eb = (edge >> (8 * e)) & 15u;
+                    if (!eb) continue;
+                    T d1[3][3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) { d1[c][0] = LN::get(dF[c][0], e); d1[c][1] = LN::get(dF[c][1], e); d1[c][2] = T(0); }
+                    face_fix<T, BW, CSX>(fr + e, eb, d1);
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) { LN::set(dF[c][0], e, d1[c][0]); LN::set(dF[c][1], e, d1[c][1]); }
+                }
             }
 #pragma unroll
             for (int c = 0; c < 3; ++c) dF[c][c] += twoh[c];
-            T n0[3];
+            V n0[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
-                n0[c] = dF[c1][1] * dF[c2][2] - dF[c2][1] * dF[c1][2];
+                n0[c] = fma(dF[c1][1], dF[c2][2], -(dF[c2][1] * dF[c1][2]));
             }
-            const T D = dF[0][0] * n0[0] + dF[1][0] * n0[1] + dF[2][0] * n0[2];
-            ok = ok && (positive_finite(D) || !dom);
-            const T inv = fast_rcp(D);
+            const V D = fma(dF[0][0], n0[0], fma(dF[1][0], n0[1], dF[2][0] * n0[2]));
+#pragma unroll
+            for (int e = 0; e < NV; ++e) ok = ok && (positive_finite(LN::get(D, e)) || !dom[e]);
+            const V inv = LN::rcp(D);
             // dF b first, the division last: the nine products do not wait for the reciprocal's Newton chain
 #pragma unroll
-            for (int c = 0; c < 3; ++c) Bp[c] = (dF[c][0] * bq[0] + dF[c][1] * bq[1] + dF[c][2] * bq[2]) * inv;
+            for (int c = 0; c < 3; ++c) Bp[c] = fma(dF[c][0], bq[0], fma(dF[c][1], bq[1], dF[c][2] * bq[2])) * inv;
             T* d = pB + Q * L::BSLOT;
-            d[0] = Bp[0];
-            d[BCS] = Bp[1];
-            d[2 * BCS] = Bp[2];
+            LN::st(d, Bp[0]);
+            LN::st(d + BCS, Bp[1]);
+            LN::st(d + 2 * BCS, Bp[2]);
             if constexpr (TILE) {
-                sh[Q & 1] = (p > 0 && p < nz - 1 && in_xy) ? a.dtg * inv : T(0);
+                V sn = LN::bc(a.dtg) * inv;
+                const bool kin = p > 0 && p < nz - 1;
+#pragma unroll
+                for (int e = 0; e < NV; ++e)
+                    if (!(kin && in_xy[e])) LN::set(sn, e, T(0));
+                sh[Q & 1] = sn;
                 uint32_t v0[C0W], v1[C1W];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -269,18 +329,12 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 W32::put(v0 + 6 * WN, n0[0]);
                 W32::put(v0 + 7 * WN, n0[1]);
                 W32::put(v1 + 3 * WN, n0[2]);
-#ifdef MR_X_TMEM
-                W32::put(v1 + 4 * WN, x1[0]);
-                W32::put(v1 + 5 * WN, x1[1]);
-                W32::put(v1 + 6 * WN, x1[2]);
-                W32::put(v1 + 7 * WN, T(0));
-#endif
                 tmem::st<C0W>(tm0 + (Q & 1) * REC, v0);
                 tmem::st<C1W>(tm0 + (Q & 1) * REC + C0W, v1);
             }
         } else if (!TILE && has_node) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) x1[c] = fr[c * CSX];
+            for (int c = 0; c < 3; ++c) x1[c] = LN::ld(fr + c * CSX);
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar + 8u * Q);                   // this warp's part of B(p) is in shared memory
@@ -294,29 +348,20 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             tmem::ld<C0W>(tm0 + ((Q + 1) & 1) * REC, w0);
             tmem::ld<C1W>(tm0 + ((Q + 1) & 1) * REC + C0W, w1);
             const T* g = pB + QM1 * L::BSLOT;
-#ifdef MR_BC_SMEM
-            const T Bc[3] = { g[0], g[BCS], g[2 * BCS] };
-#else
-            const T(&Bc)[3] = Bh[QM1];
-#endif
-#ifndef MR_BM_REG
+            const V(&Bc)[3] = Bh[QM1];
             // own B(p-2) back from its shared plane (intact until A(p+2)): cheaper than six more registers carried
             const T* gm = pB + QM2 * L::BSLOT;
-            const T Bm[3] = { gm[0], gm[BCS], gm[2 * BCS] };
-#else
-            const T(&Bm)[3] = Bh[QM2];
-#endif
-            T dBi[3], dBj[3], dBk[3];
+            V dBi[3], dBj[3], dBk[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const T* gc = g + c * BCS;
-                dBi[c] = gc[1] - gc[-1];
-                dBj[c] = gc[BBW] - gc[-BBW];
-                dBk[c] = Bp[c] - Bm[c];
+                dBi[c] = LN::di(gc, Bc[c]);
+                dBj[c] = LN::ld(gc + BBW) - LN::ld(gc - BBW);
+                dBk[c] = Bp[c] - LN::ld(gm + c * BCS);
             }
             tmem::wait_ld(w0);
             tmem::wait_ld(w1);
-            T c0[3], c1[3], c2[3], n0[3], n1[3], n2[3], DJ[3], uu[3];
+            V c0[3], c1[3], c2[3], n0[3], n1[3], n2[3], DJ[3], uu[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 c0[c] = W32::get(w0 + c * WN);
@@ -335,21 +380,17 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             if constexpr (DIAG) {
                 if (p > k0) diag_node(p - 1, c0, n0, Bc, uu);
             } else {
-                const T s = sh[(Q + 1) & 1];
-                T x[3];
+                const V s = sh[(Q + 1) & 1];
+                V x[3];
 #pragma unroll
-#ifdef MR_X_TMEM
-                for (int c = 0; c < 3; ++c) x[c] = fma(s, uu[c], W32::get(w1 + (4 + c) * WN));
-#else
                 for (int c = 0; c < 3; ++c) x[c] = RHS ? s * uu[c] : fma(s, uu[c], xp[c]);
-#endif
-#ifndef MR_NOXCHK
-                ok = ok && is_finite(x[0] + x[1] + x[2]);
-#endif
-                if (st && p > k0) {
-                    po[0] = x[0];
-                    po[a.comp] = x[1];
-                    po[2 * a.comp] = x[2];
+                const V xs = x[0] + x[1] + x[2];
+#pragma unroll
+                for (int e = 0; e < NV; ++e) ok = ok && is_finite(LN::get(xs, e));
+                if (any_st && p > k0) {
+                    store_nodes(po, x[0]);
+                    store_nodes(po + a.comp, x[1]);
+                    store_nodes(po + 2 * a.comp, x[2]);
                 }
                 po += a.plane;
             }
@@ -381,8 +422,8 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             tmem::ld<C1W>(tm0 + (ql & 1) * REC + C0W, w1);
             tmem::wait_ld(w0);
             tmem::wait_ld(w1);
-            T c0[3], n0[3], Bt[3];
-            const T zero[3] = { T(0), T(0), T(0) };
+            V c0[3], n0[3], Bt[3];
+            const V zero[3] = { LN::bc(T(0)), LN::bc(T(0)), LN::bc(T(0)) };
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 c0[c] = W32::get(w0 + c * WN);
@@ -392,10 +433,10 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             n0[1] = W32::get(w0 + 7 * WN);
             n0[2] = W32::get(w1 + 3 * WN);
             diag_node(nz - 1, c0, n0, Bt, zero);
-        } else if (st) {
+        } else if (any_st) {
             T* pl = out + (long long)(nz - 1) * a.plane + (long long)gj * a.pitch + gi;
 #pragma unroll
-            for (int c = 0; c < 3; ++c) pl[c * a.comp] = RHS ? T(0) : (ql & 1) ? xh[1][c] : xh[0][c];
+            for (int c = 0; c < 3; ++c) store_nodes(pl + c * a.comp, RHS ? LN::bc(T(0)) : (ql & 1) ? xh[1][c] : xh[0][c]);
         }
     }
     if (!ok) atomicOr(a.flag, FLAG_NUMERIC);
@@ -444,7 +485,8 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
         *why = "cuTensorMapEncodeTiled failed";
         return false;
     }
-    p->tiles_x = (g.nx + Ld::TX - 1) / Ld::TX;
+    const int tx = f64 ? Ld::TX : Lf::TX;
+    p->tiles_x = (g.nx + tx - 1) / tx;
     p->tiles_y = (g.ny + Ld::TY - 1) / Ld::TY;
     p->smem_bytes = f64 ? Ld::BYTES : Lf::BYTES;
     cudaError_t e = cudaSuccess;
