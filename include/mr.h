@@ -55,7 +55,8 @@ typedef enum {
     MR_BC_LINE_TIED = 0, /* u = 0 and B.n fixed on the face (:147) */
     MR_BC_PERIODIC = 1   /* Eqs. 2.12-2.14 (:147-164): every node of the axis is an inner point, nodes at lo + idx*h,
                             period n*h = (hi - lo) + h; the ghost nodes are x(-1) = x(n-1) - n*h e_a, x(n) = x(0) + n*h e_a
-                            and B(X,0) must be periodic.  Runs on the global-memory kernels (csrc/mr_generic.cuh). */
+                            and B(X,0) must be periodic.  The ghost nodes live in the padded arrays of the workspace (two
+                            planes / rows, 16 bytes of columns either side of a periodic axis), refreshed after every pass. */
 } mr_bc;
 
 typedef enum { MR_F64 = 0, MR_F32 = 1 } mr_dtype;
@@ -68,7 +69,7 @@ typedef struct {
     mr_bc bc[3];            /* per logical axis (both faces) */
     double gamma;           /* > 0; Eq. 1.5, the paper uses 1 (:55) */
     mr_dtype dtype;         /* storage and arithmetic type of the state; reductions always accumulate in fp64 */
-    void* workspace;        /* device pointer, >= mr_workspace_bytes(), 256-byte aligned, caller-owned */
+    void* workspace;        /* device pointer, >= mr_workspace_bytes_bc(grid, dtype, bc), 256-byte aligned, caller-owned */
     size_t workspace_bytes;
     void* stream;           /* cudaStream_t (0 = legacy default stream), caller-owned */
 } mr_boundary;
@@ -84,8 +85,11 @@ typedef struct {
 
 /* Bytes of device workspace mr_create needs for this grid and dtype (0 if the arguments are invalid).
  * Holds the double-buffered state, the pre-scaled B(X,0), a staging buffer for the *_host calls and the
- * reduction partials; about 4 fields = 12*nx*ny*nz elements.  Pure host arithmetic, needs no GPU. */
+ * reduction partials; about 4 fields = 12*nx*ny*nz elements.  Pure host arithmetic, needs no GPU.
+ * mr_workspace_bytes: all six faces line-tied.  mr_workspace_bytes_bc: bc[3] = the mr_bc of the x, y, z axes; a periodic
+ * axis adds its ghost layers (two planes / rows, 16 bytes of columns either side) to every field. */
 size_t mr_workspace_bytes(const mr_grid* grid, mr_dtype dtype);
+size_t mr_workspace_bytes_bc(const mr_grid* grid, mr_dtype dtype, const int32_t* bc);
 
 /* Create a context on the current CUDA device; the state is initialised to x = X, so a run that starts on
  * the reference grid needs no mr_set_x.
@@ -134,7 +138,8 @@ mr_status mr_rhs(mr_ctx* ctx, mr_operator op, void* u_dev);
 
 /* ---- section 2.4 (:131-143): adaptive Cash-Karp RK5(4) with the step control of Eq. 2.11 -------------------------
  * Needs a second caller-owned device buffer for the six stage velocities and the stage state (7 fields), bound once. */
-size_t mr_adaptive_workspace_bytes(const mr_grid* grid, mr_dtype dtype);
+size_t mr_adaptive_workspace_bytes(const mr_grid* grid, mr_dtype dtype);                 /* all faces line-tied */
+size_t mr_adaptive_workspace_bytes_bc(const mr_grid* grid, mr_dtype dtype, const int32_t* bc);
 mr_status mr_bind_adaptive_workspace(mr_ctx* ctx, void* workspace_dev, size_t bytes);
 
 typedef struct {

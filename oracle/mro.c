@@ -597,12 +597,15 @@ int mro_cash_karp_trial(long long m, const double* y, double dt, mro_rhs_fn f, v
 /*
  * Step control of PAPER.md:139-143: returns 1 if the trial step is accepted (Lambda <= Lambda0), 0 if it is
  * rejected, and writes the step length to use next: Eq. 2.11 dt' = dt |Lambda0/Lambda|^0.2 after a rejection or
- * when Lambda < Lambda0/2 (growth capped at 5 dt, Lambda may vanish), dt otherwise.
+ * when Lambda < Lambda0/2 (growth capped at 5 dt, Lambda may vanish), dt otherwise.  A retry after a rejection is at
+ * most 0.9 dt (reading Q22): Eq. 2.11 alone has a fixed point just above Lambda0, where the factor rounds to 1
+ * and the same trial would be repeated for ever (met on the IsoHelix run of Table 4.1: Lambda = 1.0000000000000002e-8).
  */
 int mro_step_control(double dt, double lambda, double lambda0, double* dt_next)
 {
     if (lambda > lambda0 || isnan(lambda)) {
-        *dt_next = isnan(lambda) ? 0.5 * dt : dt * pow(fabs(lambda0 / lambda), 0.2);
+        const double f = isnan(lambda) ? 0.5 : pow(fabs(lambda0 / lambda), 0.2);
+        *dt_next = dt * (f < 0.9 ? f : 0.9);
         return 0;
     }
     if (lambda < 0.5 * lambda0) {

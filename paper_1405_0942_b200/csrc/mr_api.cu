@@ -27,21 +27,29 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 struct Layout {
     int pitch;
     long long plane, comp;
+    int ghost[3];         // ghost layers either side of a periodic axis (0 on a line-tied one), DESIGN.md "Data layout"
+    long long shift;      // element offset of the node (0, 0, 0) inside a padded field
     size_t field_bytes;   // one padded 3-component field
     size_t stage_bytes;   // one dense 3-component field
     size_t off_xi[2], off_b, off_stage, off_partials, off_diag, off_flag, total;
     size_t adaptive_total;   // the second workspace: 7 padded fields
 };
 
-bool make_layout(const mr_grid* g, mr_dtype dt, Layout* L)
+// per = which axes are periodic (null = none)
+bool make_layout(const mr_grid* g, mr_dtype dt, const int* per, Layout* L)
 {
     if (!g) return false;
     if (g->nx < 5 || g->ny < 5 || g->nz < 5 || g->nx > 4096 || g->ny > 4096 || g->nz > 4096) return false;
     if (dt != MR_F64 && dt != MR_F32) return false;
     const size_t es = dt == MR_F64 ? 8 : 4;
-    L->pitch = (g->nx + 15) / 16 * 16;
-    L->plane = (long long)L->pitch * g->ny;
-    L->comp = L->plane * g->nz;
+    // a periodic axis carries its ghost nodes in the array: 2 planes / rows, 16 bytes of columns (the x halo of the TMA boxes)
+    L->ghost[0] = (per && per[0]) ? (int)(16 / es) : 0;
+    L->ghost[1] = (per && per[1]) ? 2 : 0;
+    L->ghost[2] = (per && per[2]) ? 2 : 0;
+    L->pitch = (g->nx + 2 * L->ghost[0] + 15) / 16 * 16;
+    L->plane = (long long)L->pitch * (g->ny + 2 * L->ghost[1]);
+    L->comp = L->plane * (g->nz + 2 * L->ghost[2]);
+    L->shift = (long long)L->ghost[2] * L->plane + (long long)L->ghost[1] * L->pitch + L->ghost[0];
     L->field_bytes = align_up((size_t)(3 * L->comp) * es, kAlign);
     L->stage_bytes = align_up((size_t)3 * g->nx * g->ny * g->nz * es, kAlign);
     size_t o = 0;
@@ -87,13 +95,19 @@ struct mr_ctx {
     StreamPlan plan_mim;   // the streaming kernel of the mimetic operator (mr_sym.cuh)
     std::string err;
 
-    void* xi(int w) const { return ws + L.off_xi[w]; }
-    void* b() const { return ws + L.off_b; }
+    // a padded field starts at *_raw (what the tensor maps and the elementwise kernels span); the kernels that index by
+    // node get the address of the node (0, 0, 0)
+    size_t node0() const { return (size_t)L.shift * esize(); }
+    void* xi_raw(int w) const { return ws + L.off_xi[w]; }
+    void* b_raw() const { return ws + L.off_b; }
+    void* xi(int w) const { return ws + L.off_xi[w] + node0(); }
+    void* b() const { return ws + L.off_b + node0(); }
     void* stage() const { return ws + L.off_stage; }
     DiagPartial* partials() const { return reinterpret_cast<DiagPartial*>(ws + L.off_partials); }
     DiagPartial* diag_out() const { return reinterpret_cast<DiagPartial*>(ws + L.off_diag); }
     int* flag() const { return reinterpret_cast<int*>(ws + L.off_flag); }
-    void* kbuf(int s) const { return aws + (size_t)s * L.field_bytes; }      // s = 0..5: k_1..k_6, 6: the stage state
+    void* kbuf_raw(int s) const { return aws + (size_t)s * L.field_bytes; }  // s = 0..5: k_1..k_6, 6: the stage state
+    void* kbuf(int s) const { return aws + (size_t)s * L.field_bytes + node0(); }
     size_t esize() const { return dtype == MR_F64 ? 8 : 4; }
     size_t dense_bytes() const { return (size_t)3 * grid.nx * grid.ny * grid.nz * esize(); }
 };
@@ -156,23 +170,34 @@ void ensure_plans(mr_ctx* c)
     sg.nx = c->grid.nx; sg.ny = c->grid.ny; sg.nz = c->grid.nz;
     sg.pitch = c->L.pitch; sg.plane = c->L.plane; sg.comp = c->L.comp;
     for (int a = 0; a < 3; ++a) sg.twoh[a] = 2.0 * c->h[a];
+    for (int a = 0; a < 3; ++a) { sg.ghost[a] = c->L.ghost[a]; sg.per[a] = c->per[a]; }
     std::string why;
-    if (c->any_periodic) {       // the TMA boxes rely on zero fill outside the grid: line-tied faces only
-        c->plan_dir.usable = c->plan_mim.usable = false;
-        return;
-    }
-    if (!build_direct_plan(&c->plan_dir, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+    if (!build_direct_plan(&c->plan_dir, sg, c->dtype == MR_F64, c->xi_raw(0), c->xi_raw(1), c->b_raw(), c->sm_count, &why)) {
         c->plan_dir.usable = false;
         c->plan_dir.why = why;
     }
-    if (!build_sym_plan(&c->plan_mim, sg, c->dtype == MR_F64, c->xi(0), c->xi(1), c->b(), c->sm_count, &why)) {
+    if (!build_sym_plan(&c->plan_mim, sg, c->dtype == MR_F64, c->xi_raw(0), c->xi_raw(1), c->b_raw(), c->sm_count, &why)) {
         c->plan_mim.usable = false;
         c->plan_mim.why = why;
     }
     if (c->aws) {
-        if (c->plan_mim.usable && !sym_bind_stage(&c->plan_mim, c->kbuf(6))) c->plan_mim.usable = false;
-        if (c->plan_dir.usable && !direct_bind_stage(&c->plan_dir, c->kbuf(6))) c->plan_dir.usable = false;
+        if (c->plan_mim.usable && !sym_bind_stage(&c->plan_mim, c->kbuf_raw(6))) c->plan_mim.usable = false;
+        if (c->plan_dir.usable && !direct_bind_stage(&c->plan_dir, c->kbuf_raw(6))) c->plan_dir.usable = false;
     }
+}
+
+// keep the ghost layers of the periodic axes of a padded field equal to the nodes they wrap to (`field` = its node (0,0,0))
+template <typename T>
+void wrap_ghosts(mr_ctx* c, void* field)
+{
+    if (!c->any_periodic) return;
+    const int* gh = c->L.ghost;
+    const long long px = c->grid.nx + 2 * gh[0], py = c->grid.ny + 2 * gh[1];
+    const long long n = 2LL * gh[2] * py * px + (long long)c->grid.nz * 2 * gh[1] * px + (long long)c->grid.nz * c->grid.ny * 2 * gh[0];
+    long long blocks = (n + 255) / 256;
+    if (blocks > (long long)c->sm_count * 16) blocks = (long long)c->sm_count * 16;
+    k_wrap<T><<<(unsigned)blocks, 256, 0, c->stream>>>(static_cast<T*>(field), grid_params<T>(c), gh[0], gh[1], gh[2]);
+    c->launches++;
 }
 
 bool streaming(mr_ctx* c, mr_operator op)
@@ -191,6 +216,7 @@ mr_status do_set_B0(mr_ctx* c, const void* B0_dev)
     k_import_B0<T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(B0_dev), static_cast<T*>(c->b()),
                                                   grid_params<T>(c), s0, s1, s2);
     c->launches++;
+    wrap_ghosts<T>(c, c->b());
     MR_CUDA(c, cudaGetLastError());
     c->have_B0 = true;
     return MR_OK;
@@ -210,6 +236,7 @@ mr_status do_set_x(mr_ctx* c, const void* src, bool as_xi)
         k_import_x<T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(src), static_cast<T*>(c->xi(other)), grid_params<T>(c),
                                                      domain_params(c), c->flag());
     c->launches++;
+    wrap_ghosts<T>(c, c->xi(other));
     MR_CUDA(c, cudaGetLastError());
     int f = 0;
     mr_status s = read_flag(c, &f);
@@ -279,6 +306,7 @@ mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
     for (int64_t s = 0; s < n; ++s) {
         mr_status st = launch_pass<T>(c, op, c->cur, c->xi(1 - c->cur), dt * c->gamma, false);
         if (st != MR_OK) return st;
+        wrap_ghosts<T>(c, c->xi(1 - c->cur));
         c->cur = 1 - c->cur;
     }
     MR_CUDA(c, cudaGetLastError());
@@ -354,27 +382,29 @@ mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* num
     static const CashKarp ck = cash_karp();
     const long long n2 = 3 * c->L.comp / 2;             // element pairs of a padded field (pitch is a multiple of 16)
     const int blocks = c->sm_count * 8 < kMaxPartialBlocks ? c->sm_count * 8 : kMaxPartialBlocks;
-    const T* x = static_cast<const T*>(c->xi(c->cur));
-    T* xs = static_cast<T*>(c->kbuf(6));
+    const T* x = static_cast<const T*>(c->xi_raw(c->cur));      // the elementwise kernels run over the whole padded fields
+    T* xs = static_cast<T*>(c->kbuf_raw(6));
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     for (int s = 0; s < 6; ++s) {
         if (s > 0) {
             StageArgs a;
             a.n = s;
-            for (int r = 0; r < 6; ++r) { a.k[r] = c->kbuf(r < s ? r : 0); a.c[r] = r < s ? h * ck.a[s][r] : 0.0; }
+            for (int r = 0; r < 6; ++r) { a.k[r] = c->kbuf_raw(r < s ? r : 0); a.c[r] = r < s ? h * ck.a[s][r] : 0.0; }
             k_rk_stage<T><<<blocks, 256, 0, c->stream>>>(x, xs, a, n2);
             c->launches++;
+            wrap_ghosts<T>(c, c->kbuf(6));                        // (the ghosts of the k_r are not kept)
         }
         mr_status st = launch_pass<T>(c, op, s == 0 ? c->cur : 2, c->kbuf(s), c->gamma, true);
         if (st != MR_OK) return st;
     }
     StageArgs b5, db;
     b5.n = db.n = 6;
-    for (int r = 0; r < 6; ++r) { b5.k[r] = db.k[r] = c->kbuf(r); b5.c[r] = h * ck.b5[r]; db.c[r] = h * ck.db[r]; }
+    for (int r = 0; r < 6; ++r) { b5.k[r] = db.k[r] = c->kbuf_raw(r); b5.c[r] = h * ck.b5[r]; db.c[r] = h * ck.db[r]; }
     double* partial = reinterpret_cast<double*>(c->partials());
-    k_rk_final<T><<<blocks, 256, 0, c->stream>>>(x, static_cast<T*>(c->xi(1 - c->cur)), b5, db, n2, partial);
+    k_rk_final<T><<<blocks, 256, 0, c->stream>>>(x, static_cast<T*>(c->xi_raw(1 - c->cur)), b5, db, n2, partial);
     k_max_final<<<1, 256, 0, c->stream>>>(partial, blocks, reinterpret_cast<double*>(c->diag_out()));
     c->launches += 2;
+    wrap_ghosts<T>(c, c->xi(1 - c->cur));
     MR_CUDA(c, cudaGetLastError());
     MR_CUDA(c, cudaMemcpyAsync(lambda, c->diag_out(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     return read_flag(c, numeric);
@@ -384,7 +414,9 @@ mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* num
 bool step_control(double dt, double lambda, double lambda0, double* dt_next)
 {
     if (lambda > lambda0 || lambda != lambda) {
-        *dt_next = lambda != lambda ? 0.5 * dt : dt * std::pow(std::fabs(lambda0 / lambda), 0.2);
+        // (a retry is at most 0.9 dt: just above lambda0 the factor of Eq. 2.11 rounds to 1 and the trial would repeat for ever)
+        const double f = lambda != lambda ? 0.5 : std::pow(std::fabs(lambda0 / lambda), 0.2);
+        *dt_next = dt * (f < 0.9 ? f : 0.9);
         return false;
     }
     if (lambda < 0.5 * lambda0) {
@@ -489,13 +521,38 @@ mr_status do_sigma(mr_ctx* c, const void* x_ref, const void* B_ref, double* sx, 
 extern "C" size_t mr_workspace_bytes(const mr_grid* grid, mr_dtype dtype)
 {
     Layout L;
-    return make_layout(grid, dtype, &L) ? L.total : 0;
+    return make_layout(grid, dtype, nullptr, &L) ? L.total : 0;
+}
+
+namespace {
+bool periodic_axes(const int32_t* bc, int (&per)[3])
+{
+    for (int a = 0; a < 3; ++a) {
+        if (!bc || (bc[a] != MR_BC_LINE_TIED && bc[a] != MR_BC_PERIODIC)) return false;
+        per[a] = bc[a] == MR_BC_PERIODIC ? 1 : 0;
+    }
+    return true;
+}
+}  // namespace
+
+extern "C" size_t mr_workspace_bytes_bc(const mr_grid* grid, mr_dtype dtype, const int32_t* bc)
+{
+    Layout L;
+    int per[3];
+    return periodic_axes(bc, per) && make_layout(grid, dtype, per, &L) ? L.total : 0;
+}
+
+extern "C" size_t mr_adaptive_workspace_bytes_bc(const mr_grid* grid, mr_dtype dtype, const int32_t* bc)
+{
+    Layout L;
+    int per[3];
+    return periodic_axes(bc, per) && make_layout(grid, dtype, per, &L) ? L.adaptive_total : 0;
 }
 
 extern "C" size_t mr_adaptive_workspace_bytes(const mr_grid* grid, mr_dtype dtype)
 {
     Layout L;
-    return make_layout(grid, dtype, &L) ? L.adaptive_total : 0;
+    return make_layout(grid, dtype, nullptr, &L) ? L.adaptive_total : 0;
 }
 
 extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, const mr_boundary* boundary, mr_ctx** out)
@@ -503,9 +560,11 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
     if (out) *out = nullptr;
     if (!grid || !domain || !boundary || !out) return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: null argument");
     Layout L;
-    if (!make_layout(grid, boundary->dtype, &L))
+    if (!make_layout(grid, boundary->dtype, nullptr, &L))
         return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: each of nx, ny, nz must be in [5, 4096] and dtype MR_F64 or MR_F32");
+    int per[3] = { 0, 0, 0 };
     for (int a = 0; a < 3; ++a) {
+        per[a] = boundary->bc[a] == MR_BC_PERIODIC ? 1 : 0;
         if (!std::isfinite(domain->lo[a]) || !std::isfinite(domain->hi[a]) || !(domain->hi[a] > domain->lo[a]))
             return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: domain needs finite hi > lo on every axis");
         if (boundary->bc[a] != MR_BC_LINE_TIED && boundary->bc[a] != MR_BC_PERIODIC)
@@ -515,8 +574,9 @@ extern "C" mr_status mr_create(const mr_grid* grid, const mr_domain* domain, con
         return fail(nullptr, MR_ERR_INVALID_ARG, "mr_create: gamma must be finite and > 0");
     if (!boundary->workspace || (reinterpret_cast<uintptr_t>(boundary->workspace) % kAlign) != 0)
         return fail(nullptr, MR_ERR_WORKSPACE, "mr_create: workspace is null or not 256-byte aligned");
+    make_layout(grid, boundary->dtype, per, &L);      // (ghost layers on the periodic axes)
     if (boundary->workspace_bytes < L.total)
-        return fail(nullptr, MR_ERR_WORKSPACE, "mr_create: workspace smaller than mr_workspace_bytes()");
+        return fail(nullptr, MR_ERR_WORKSPACE, "mr_create: workspace smaller than mr_workspace_bytes_bc()");
 
     int dev = 0;
     MR_CUDA(nullptr, cudaGetDevice(&dev));
@@ -659,12 +719,12 @@ extern "C" mr_status mr_bind_adaptive_workspace(mr_ctx* ctx, void* workspace_dev
     if (!workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) % kAlign) != 0)
         return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_adaptive_workspace: workspace is null or not 256-byte aligned");
     if (bytes < ctx->L.adaptive_total)
-        return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_adaptive_workspace: smaller than mr_adaptive_workspace_bytes()");
+        return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_adaptive_workspace: smaller than mr_adaptive_workspace_bytes_bc()");
     ctx->aws = static_cast<char*>(workspace_dev);
     MR_CUDA(ctx, cudaMemsetAsync(ctx->aws, 0, ctx->L.adaptive_total, ctx->stream));       // the padding must stay finite
     if (ctx->plans_built) {
-        if (ctx->plan_mim.usable && !sym_bind_stage(&ctx->plan_mim, ctx->kbuf(6))) ctx->plan_mim.usable = false;
-        if (ctx->plan_dir.usable && !direct_bind_stage(&ctx->plan_dir, ctx->kbuf(6))) ctx->plan_dir.usable = false;
+        if (ctx->plan_mim.usable && !sym_bind_stage(&ctx->plan_mim, ctx->kbuf_raw(6))) ctx->plan_mim.usable = false;
+        if (ctx->plan_dir.usable && !direct_bind_stage(&ctx->plan_dir, ctx->kbuf_raw(6))) ctx->plan_dir.usable = false;
     }
     return MR_OK;
 }

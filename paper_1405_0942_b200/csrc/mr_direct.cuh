@@ -136,7 +136,9 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
     const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY;
     const int nz = a.nz;
     const int k0 = chunk * a.chunk_len, k1 = min(k0 + a.chunk_len, nz);
-    const int pfirst = max(k0 - 1, 0), plast = min(k1, nz - 1);        // planes this item touches
+    // a periodic axis (Eqs. 2.12-2.14) has no face: its ghost layers sit in the padded arrays, every node is an inner point
+    const bool perx = (a.per & 1) != 0, pery = (a.per & 2) != 0, perz = (a.per & 4) != 0;
+    const int pfirst = max(k0 - 1, perz ? -1 : 0), plast = min(k1, perz ? nz : nz - 1);        // planes this item touches
     const T twoh[3] = { a.twoh[0], a.twoh[1], a.twoh[2] };
 
     // ---- TMA producer: lane 0 of the last warp; one mbarrier per slot covers the xi box and the b box ----
@@ -146,8 +148,8 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
         for (const int last = min(upto, plast); next <= last; ++next) {
             const uint32_t s = (uint32_t)((next - pfirst) % R);
             ptx::mbar_expect_tx(bar + 8u * s, 2u * L::BOX_BYTES);
-            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOT * sizeof(T)), &map_in, i0 - L::HX, j0 - 1, next, 0, bar + 8u * s);
-            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOT * sizeof(T)), &map_b, i0 - L::HX, j0 - 1, next, 0, bar + 8u * s);
+            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOT * sizeof(T)), &map_in, i0 - L::HX + a.ox, j0 - 1 + a.oy, next + a.oz, 0, bar + 8u * s);
+            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOT * sizeof(T)), &map_b, i0 - L::HX + a.ox, j0 - 1 + a.oy, next + a.oz, 0, bar + 8u * s);
         }
     };
     if (producer) {
@@ -159,7 +161,7 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
 
     const int gi = i0 + lane, gj = j0 + warp;
     const bool in_dom = gi < a.nx && gj < a.ny;
-    const bool in_xy = gi > 0 && gi < a.nx - 1 && gj > 0 && gj < a.ny - 1;
+    const bool in_xy = in_dom && (perx || (gi > 0 && gi < a.nx - 1)) && (pery || (gj > 0 && gj < a.ny - 1));
     const int o = (warp + 1) * BW + lane + L::HX;                      // this node inside a box
     auto wait_plane = [&](int p) { const int q = p - pfirst; ptx::mbar_wait(bar + 8u * (uint32_t)(q % R), (uint32_t)((q / R) & 1)); };
     for (int p = pfirst; p <= min(k0, plast); ++p) wait_plane(p);
@@ -177,7 +179,7 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
         const T* xc = sx + sc * L::SLOT + o;
         T x[3] = { xc[0], xc[CS], xc[2 * CS] };
         if (RHS) x[0] = x[1] = x[2] = T(0);
-        const bool inner = in_xy && k > 0 && k < nz - 1;
+        const bool inner = in_xy && (perz || (k > 0 && k < nz - 1));
         if (inner) {
             T J[3], B[3], u[3], D;
             direct_J_smem<T, BW, CS>(sx + sm * L::SLOT + o, xc, sx + sp * L::SLOT + o, sb + sm * L::SLOT + o, sb + sc * L::SLOT + o,
@@ -248,9 +250,9 @@ inline bool build_direct_plan(StreamPlan* p, const StreamGeom& g, bool f64, void
     p->usable = false;
     p->f64 = f64;
     p->g = g;
-    p->xi[0] = xi0;
-    p->xi[1] = xi1;
-    p->b = b;
+    p->xi[0] = node_base(xi0, g, f64);      // xi0, xi1, b: the starts of the padded arrays (what the tensor maps span)
+    p->xi[1] = node_base(xi1, g, f64);
+    p->b = node_base(b, g, f64);
     p->name = f64 ? "direct_tma_f64" : "direct_tma_f32";
     const int bw = f64 ? Ld::BW : Lf::BW;
     if (!encode_map(&p->map_xi[0], f64, xi0, g, bw, kXTY + 2) || !encode_map(&p->map_xi[1], f64, xi1, g, bw, kXTY + 2) ||
@@ -285,23 +287,8 @@ inline bool direct_bind_stage(StreamPlan* p, void* xs)
 {
     const int bw = p->f64 ? DirectLayout<double, kXTY, kXR>::BW : DirectLayout<float, kXTY, kXR>::BW;
     if (!encode_map(&p->map_xi[2], p->f64, xs, p->g, bw, kXTY + 2)) return false;
-    p->xi[2] = xs;
+    p->xi[2] = node_base(xs, p->g, p->f64);
     return true;
-}
-
-template <typename T>
-inline StreamArgs<T> direct_args(const StreamPlan& p, T dtg, int* flag)
-{
-    StreamArgs<T> a;
-    a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
-    a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
-    for (int c = 0; c < 3; ++c) a.twoh[c] = (T)p.g.twoh[c];
-    a.dtg = dtg;
-    a.tiles_x = p.tiles_x;
-    a.ntiles = p.tiles_x * p.tiles_y;
-    a.chunk_len = p.chunk_len;
-    a.flag = flag;
-    return a;
 }
 
 // one step / one right-hand side of the state in the plan's buffer `cur` (see launch_sym_step)
@@ -309,7 +296,7 @@ template <typename T>
 inline cudaError_t launch_direct_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream, bool rhs = false, void* out = nullptr)
 {
     using L = DirectLayout<T, kXTY, kXR>;
-    const StreamArgs<T> a = direct_args<T>(p, dtg, flag);
+    const StreamArgs<T> a = stream_args<T>(p, dtg, flag);
     T* o = static_cast<T*>(out ? out : p.xi[1 - cur]);
     const int grid = a.ntiles * p.nchunks;
     if (rhs) k_step_direct<T, kXTY, kXR, 2><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, o, a);
@@ -322,7 +309,7 @@ template <typename T>
 inline cudaError_t launch_direct_diag(const StreamPlan& p, int cur, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
 {
     using L = DirectLayout<T, kXTY, kXR>;
-    const StreamArgs<T> a = direct_args<T>(p, (T)0, flag);
+    const StreamArgs<T> a = stream_args<T>(p, (T)0, flag);
     *nblocks = a.ntiles * p.nchunks;
     k_step_direct<T, kXTY, kXR, 1><<<*nblocks, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();

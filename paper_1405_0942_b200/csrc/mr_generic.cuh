@@ -89,6 +89,43 @@ __global__ void k_export_padded(const T* __restrict__ src, T* __restrict__ dst, 
     for (int c = 0; c < 3; ++c) dst[c * N + q] = src[c * g.comp + p];
 }
 
+// Ghost layers of the periodic axes (Eqs. 2.12-2.14; reading Q12): in the displacement xi = x - X, and in b, the
+// ghost node of index idx < 0 or idx >= n is the node idx mod n.  `f` points at the node (0, 0, 0) of a padded field whose
+// periodic axes carry gx / gy / gz layers either side; every ghost node copies its three components from the node it wraps
+// to.  The streaming kernels read their halos out of these layers; one thread per ghost node, x fastest.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_wrap(T* __restrict__ f, GridP<T> g, int gx, int gy, int gz)
+{
+    const long long px = g.nx + 2 * gx, py = g.ny + 2 * gy;
+    const long long nA = 2LL * gz * py * px;                 // the z slabs (all rows, all columns)
+    const long long nB = (long long)g.nz * 2 * gy * px;      // the y slabs of the planes 0 .. nz-1
+    const long long nC = (long long)g.nz * g.ny * 2 * gx;    // the x slabs of the rows 0 .. ny-1 of those planes
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nA + nB + nC; q += (long long)gridDim.x * blockDim.x) {
+        long long i, j, k, r = q;
+        if (r < nA) {
+            i = r % px - gx; r /= px;
+            j = r % py - gy; r /= py;
+            k = r < gz ? r - gz : g.nz + (r - gz);
+        } else if ((r -= nA) < nB) {
+            i = r % px - gx; r /= px;
+            const long long jj = r % (2 * gy); r /= 2 * gy;
+            j = jj < gy ? jj - gy : g.ny + (jj - gy);
+            k = r;
+        } else {
+            r -= nB;
+            const long long ii = r % (2 * gx); r /= 2 * gx;
+            i = ii < gx ? ii - gx : g.nx + (ii - gx);
+            j = r % g.ny;
+            k = r / g.ny;
+        }
+        const long long si = (i % g.nx + g.nx) % g.nx, sj = (j % g.ny + g.ny) % g.ny, sk = (k % g.nz + g.nz) % g.nz;
+        const long long dst = k * g.plane + j * g.pitch + i, src = sk * g.plane + sj * g.pitch + si;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) f[c * g.comp + dst] = f[c * g.comp + src];
+    }
+}
+
 // B0 (dense) -> b_a = scale_a * B0_a (padded), scale_a = 4 h_b h_c
 template <typename T>
 __global__ void k_import_B0(const T* __restrict__ B0, T* __restrict__ b, GridP<T> g, double s0, double s1, double s2)

@@ -4,7 +4,9 @@
 // encoding and z-chunking.  Work item of every streaming kernel = (xy tile of 32 x 16 nodes, chunk of z-planes): a CTA
 // marches along k while the TMA unit streams, per plane, the box of the displacement xi and of the pre-scaled b (4-D
 // tiled maps over [c][k][j][i]) into shared-memory rings; out-of-domain parts of a box are zero-filled by the TMA
-// unit, so domain edges need no address logic.
+// unit, so line-tied domain edges need no address logic.  A periodic axis (Eqs. 2.12-2.14) carries ghost layers in the
+// padded array itself (mr_api.cu keeps them equal to the wrapped nodes, k_wrap): the maps span the padded extent, the box
+// coordinates are shifted by the ghost width, and a box over the edge reads the neighbours through the wrap.
 #pragma once
 #include <cuda.h>
 
@@ -20,6 +22,9 @@ struct StreamGeom {
     int nx, ny, nz, pitch;
     long long plane, comp;
     double twoh[3];
+    int ghost[3];         // ghost layers in front of (and behind) the nodes of a periodic axis, 0 on a line-tied one
+    int per[3];
+    long long shift() const { return (long long)ghost[2] * plane + (long long)ghost[1] * pitch + ghost[0]; }   // node (0,0,0)
 };
 
 template <typename T>
@@ -30,6 +35,8 @@ struct StreamArgs {
     T twoh[3];
     T dtg;
     int tiles_x, ntiles, chunk_len;
+    int ox, oy, oz;       // box coordinate of the node (0, 0, 0) in the tensor maps (= the ghost widths)
+    int per;              // bit a: axis a is periodic (no face, no one-sided difference, every node an inner point)
     int* flag;
 };
 
@@ -203,7 +210,8 @@ inline bool encode_map(CUtensorMap* m, bool f64, void* base, const StreamGeom& g
     PFN_encodeTiled enc = get_encode_fn();
     if (!enc) return false;
     const cuuint64_t es = f64 ? 8 : 4;
-    cuuint64_t dims[4] = { (cuuint64_t)g.nx, (cuuint64_t)g.ny, (cuuint64_t)g.nz, 3 };
+    // `base` is the start of the padded array (the ghost layers of a periodic axis included)
+    cuuint64_t dims[4] = { (cuuint64_t)(g.nx + 2 * g.ghost[0]), (cuuint64_t)(g.ny + 2 * g.ghost[1]), (cuuint64_t)(g.nz + 2 * g.ghost[2]), 3 };
     cuuint64_t strides[3] = { (cuuint64_t)g.pitch * es, (cuuint64_t)g.plane * es, (cuuint64_t)g.comp * es };
     cuuint32_t box[4] = { (cuuint32_t)bw, (cuuint32_t)bh, 1, 3 };
     cuuint32_t estr[4] = { 1, 1, 1, 1 };
@@ -211,6 +219,12 @@ inline bool encode_map(CUtensorMap* m, bool f64, void* base, const StreamGeom& g
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, MR_L2_PROMOTION,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
+}
+
+// the real-node base of a padded array whose storage starts at `raw`
+inline void* node_base(void* raw, const StreamGeom& g, bool f64)
+{
+    return static_cast<char*>(raw) + (size_t)g.shift() * (f64 ? 8 : 4);
 }
 
 // choose the number of z-chunks: minimise waves * (chunk_len + restart overhead) over the concurrent CTA slots
@@ -230,6 +244,24 @@ inline void choose_chunks(int ntiles, int nz, int slots, int* nchunks, int* chun
     *nchunks = bc;
     *chunk_len = (nz + bc - 1) / bc;
     *nchunks = (nz + *chunk_len - 1) / *chunk_len;
+}
+
+
+template <typename T>
+inline StreamArgs<T> stream_args(const StreamPlan& p, T dtg, int* flag)
+{
+    StreamArgs<T> a;
+    a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
+    a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
+    for (int c = 0; c < 3; ++c) a.twoh[c] = (T)p.g.twoh[c];
+    a.dtg = dtg;
+    a.tiles_x = p.tiles_x;
+    a.ntiles = p.tiles_x * p.tiles_y;
+    a.chunk_len = p.chunk_len;
+    a.ox = p.g.ghost[0]; a.oy = p.g.ghost[1]; a.oz = p.g.ghost[2];
+    a.per = (p.g.per[0] ? 1 : 0) | (p.g.per[1] ? 2 : 0) | (p.g.per[2] ? 4 : 0);
+    a.flag = flag;
+    return a;
 }
 
 }  // namespace mr

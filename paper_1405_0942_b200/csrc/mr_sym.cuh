@@ -23,6 +23,7 @@
 // are named at compile time, so the loop carries no register moves and no address arithmetic (ncu of the rolled loop:
 // 82 of its 356 instructions per node were moves, profiles/r1f_full.md).
 #pragma once
+#include <climits>
 #include <type_traits>
 
 #include "mr_generic.cuh"
@@ -76,7 +77,8 @@ inline __device__ double Lanes<double>::rcp(double d) { return fast_rcp(d); }
 
 enum : int { MODE_STEP = 0, MODE_DIAG = 1, MODE_RHS = 2 };     // xi+ = xi + dt u  |  the reduction S6  |  out = u = gamma J x B
 
-template <typename T, int MODE>
+// PER = false: all six faces line-tied (the hot path: no periodic logic is compiled in);  PER = true: at least one periodic axis
+template <typename T, int MODE, bool PER>
 __global__ void __maxnreg__(96)
 k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_b, const T* __restrict__ in,
            T* __restrict__ out, const StreamArgs<T> a)
@@ -105,10 +107,16 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int tile = blockIdx.x % a.ntiles, chunk = blockIdx.x / a.ntiles;
     const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY;
     const int nz = a.nz;
+    // a periodic axis (Eqs. 2.12-2.14) has no face: its ghost layers (two planes / rows, 16 bytes of columns either side) sit
+    // in the padded arrays, B is formed on the first ghost layer like on any halo node, and every node is an inner point
+    const bool perx = PER && (a.per & 1) != 0, pery = PER && (a.per & 2) != 0, perz = PER && (a.per & 4) != 0;
+    const int ox = PER ? a.ox : 0, oy = PER ? a.oy : 0, oz = PER ? a.oz : 0;
+    const int zface_lo = perz ? INT_MIN : 0, zface_hi = perz ? INT_MIN : nz - 1;    // the planes of the line-tied z faces
+    const int zx_lo = perz ? -2 : 0, zx_hi = perz ? nz + 1 : nz - 1;               // the xi / b planes that exist
     const int k0 = chunk * a.chunk_len, k1 = min(k0 + a.chunk_len, nz);
-    const int kend = min(k1, nz - 1);               // planes k0 .. kend-1 are finished here (and nz-1 carried through)
-    const int first_p = max(k0 - 1, 0);             // B is formed on the planes first_p .. kend
-    const int plast = min(kend + 1, nz - 1);        // last xi / b plane this item touches
+    const int kend = min(k1, zx_hi - (perz ? 1 : 0)); // planes k0 .. kend-1 are finished here (line-tied: nz-1 carried through)
+    const int first_p = max(k0 - 1, zx_lo + (perz ? 1 : 0));   // B is formed on the planes first_p .. kend
+    const int plast = min(kend + 1, zx_hi);         // last xi / b plane this item touches
     const V twoh[3] = { LN::bc(a.twoh[0]), LN::bc(a.twoh[1]), LN::bc(a.twoh[2]) };
 
     const bool pwarp = warp == NW - 1, producer = pwarp && lane == 0;
@@ -130,8 +138,8 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         const int P = first_p + r;
         if (P <= plast) {
             ptx::mbar_expect_tx(b, PLANE_BYTES);
-            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL, j0 - 2, P, 0, b);
-            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL, j0 - 1, P, 0, b);
+            ptx::tma_load_4d(sx_u32 + s * (uint32_t)(L::SLOTX * sizeof(T)), &map_in, i0 - L::HXL + ox, j0 - 2 + oy, P + oz, 0, b);
+            ptx::tma_load_4d(sb_u32 + s * (uint32_t)(L::SLOTB * sizeof(T)), &map_b, i0 - L::HXL + ox, j0 - 1 + oy, P + oz, 0, b);
         } else {
             ptx::mbar_arrive(b);
         }
@@ -163,19 +171,23 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const T* px = sx + (tj + 2) * BW + (ti + L::HXL);       // this thread in component 0 of the ring position 0 (xi, b, B)
     const T* pb = sb + (tj + 1) * BW + (ti + L::HXL);
     T* pB = sB + (tj + 1) * BBW + (ti + NV);
-    // per node e of the thread: inside the grid / on which faces (1: i = 0, 2: i = nx-1, 4: j = 0, 8: j = ny-1) / interior in xy
+    // per node e of the thread: a node or a periodic ghost (dom) / on which line-tied faces (1: i = 0, 2: i = nx-1, 4: j = 0,
+    // 8: j = ny-1) / an inner point in xy / a node this thread stores (st)
     bool dom[NV], in_xy[NV], st[NV];
     unsigned edge = 0u;                                     // bits of the node e shifted by 8 e (bits 16, 32 of `special`: the k faces)
     bool any_st = false;
-    const bool row_in = gj >= 0 && gj < a.ny;
+    const bool row_real = gj >= 0 && gj < a.ny;
+    const bool row_in = row_real || (gj >= -oy && gj < a.ny + oy);
 #pragma unroll
     for (int e = 0; e < NV; ++e) {
         const int g = gi + e;
-        dom[e] = has_node && row_in && g >= 0 && g < a.nx;
-        in_xy[e] = g > 0 && g < a.nx - 1 && gj > 0 && gj < a.ny - 1;
-        st[e] = tilew && dom[e];
+        const bool real = has_node && row_real && g >= 0 && g < a.nx;
+        dom[e] = has_node && row_in && g >= -ox && g < a.nx + ox;
+        in_xy[e] = real && (perx || (g > 0 && g < a.nx - 1)) && (pery || (gj > 0 && gj < a.ny - 1));
+        st[e] = tilew && real;
         any_st = any_st || st[e];
-        if (dom[e]) edge |= ((g == 0 ? 1u : 0u) | (g == a.nx - 1 ? 2u : 0u) | (gj == 0 ? 4u : 0u) | (gj == a.ny - 1 ? 8u : 0u)) << (8 * e);
+        if (real) edge |= ((g == 0 && !perx ? 1u : 0u) | (g == a.nx - 1 && !perx ? 2u : 0u) | (gj == 0 && !pery ? 4u : 0u) |
+                           (gj == a.ny - 1 && !pery ? 8u : 0u)) << (8 * e);
     }
 
     bool ok = true;
@@ -194,7 +206,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             xh[0][c] = LN::bc(T(0));
-            xh[1][c] = first_p > 0 ? from_global(in + c * a.comp, o) : LN::bc(T(0));     // phase 0 reads xi(first_p - 1) from xh[1]
+            xh[1][c] = first_p > zx_lo ? from_global(in + c * a.comp, o) : LN::bc(T(0)); // phase 0 reads xi(first_p - 1) from xh[1]
 #pragma unroll
             for (int q = 0; q < 4; ++q) Bh[q][c] = LN::bc(T(0));
         }
@@ -218,7 +230,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         for (int e = 0; e < NV; ++e) {
             if (!st[e]) continue;
             const int g = gi + e;
-            const double zxy = ((g == 0 || g == a.nx - 1) ? 0.5 : 1.0) * ((gj == 0 || gj == a.ny - 1) ? 0.5 : 1.0);   // Eq. 3.13
+            const double zxy = ((edge >> (8 * e)) & 3u ? 0.5 : 1.0) * ((edge >> (8 * e)) & 12u ? 0.5 : 1.0);          // Eq. 3.13
             double D = 0.0, b2 = 0.0, u2 = 0.0;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
@@ -226,7 +238,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 b2 += (double)LN::get(B[c], e) * (double)LN::get(B[c], e);
                 u2 += (double)LN::get(uu[c], e) * (double)LN::get(uu[c], e);
             }
-            const bool kface = k == 0 || k == nz - 1;
+            const bool kface = k == zface_lo || k == zface_hi;
             DiagPartial v = { zxy * (kface ? 0.5 : 1.0) * b2 * D, 0.0, 0.0, D };
             if (in_xy[e] && !kface) {
                 const double fm = sqrt(u2) / D;
@@ -240,7 +252,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     if (!pwarp) {        // the planes first_p, first_p + 1 and, for the one-sided difference on the bottom face, 2
         ptx::mbar_wait(bar + 8u, 0u);
         ptx::mbar_wait(bar + 16u, 0u);
-        if (first_p == 0) ptx::mbar_wait(bar + 24u, 0u);
+        if (first_p == zface_lo) ptx::mbar_wait(bar + 24u, 0u);
     }
     int p = first_p;
     uint32_t gpar = 0u;                                      // parity of the group of four planes
@@ -267,7 +279,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 dF[c][2] = LN::ld(f2p + c * CSX) - xp[c];
                 bq[c] = LN::ld(pb + S0 * L::SLOTB + c * CSB);
             }
-            const unsigned special = edge | (p == 0 ? 16u : 0u) | (p == nz - 1 ? 32u : 0u);
+            const unsigned special = edge | (p == zface_lo ? 16u : 0u) | (p == zface_hi ? 32u : 0u);
             if (special) {
                 if (special & 16u) {            // bottom face: -3 x(0) + 4 x(1) - x(2)
                     const T* f3 = px + S2 * L::SLOTX;
@@ -314,7 +326,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             LN::st(d + 2 * BCS, Bp[2]);
             if constexpr (TILE) {
                 V sn = LN::bc(a.dtg) * inv;
-                const bool kin = p > 0 && p < nz - 1;
+                const bool kin = p != zface_lo && p != zface_hi;
 #pragma unroll
                 for (int e = 0; e < NV; ++e)
                     if (!(kin && in_xy[e])) LN::set(sn, e, T(0));
@@ -413,7 +425,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     if (tilew) run(std::true_type{});
     else if (!pwarp) run(std::false_type{});
 
-    if (k1 == nz && tilew) {   // the top plane (line-tied) is carried through / enters the energy sum
+    if (k1 == nz && tilew && !perz) {   // the top plane (line-tied) is carried through / enters the energy sum
         const int ql = (nz - 1 - first_p) & 3;
         if constexpr (DIAG) {
             uint32_t w0[C0W], w1[C1W];
@@ -467,6 +479,17 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 
 // ----------------------------------------------------------------------------------------------- host side
 
+template <typename T>
+using SymKernel = void (*)(const CUtensorMap, const CUtensorMap, const T*, T*, const StreamArgs<T>);
+
+// the instantiation for a mode and for "some axis is periodic"
+template <typename T>
+inline SymKernel<T> sym_kernel(int mode, bool per)
+{
+    if (per) return mode == MODE_STEP ? k_step_sym<T, MODE_STEP, true> : mode == MODE_DIAG ? k_step_sym<T, MODE_DIAG, true> : k_step_sym<T, MODE_RHS, true>;
+    return mode == MODE_STEP ? k_step_sym<T, MODE_STEP, false> : mode == MODE_DIAG ? k_step_sym<T, MODE_DIAG, false> : k_step_sym<T, MODE_RHS, false>;
+}
+
 inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* xi0, void* xi1, void* b, int sm_count,
                            std::string* why)
 {
@@ -475,9 +498,9 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
     p->usable = false;
     p->f64 = f64;
     p->g = g;
-    p->xi[0] = xi0;
-    p->xi[1] = xi1;
-    p->b = b;
+    p->xi[0] = node_base(xi0, g, f64);      // xi0, xi1, b: the starts of the padded arrays (what the tensor maps span)
+    p->xi[1] = node_base(xi1, g, f64);
+    p->b = node_base(b, g, f64);
     p->name = f64 ? "sym_tmem_f64" : "sym_tmem_f32";
     const int bw = f64 ? Ld::BW : Lf::BW;
     if (!encode_map(&p->map_xi[0], f64, xi0, g, bw, Ld::TY + 4) || !encode_map(&p->map_xi[1], f64, xi1, g, bw, Ld::TY + 4) ||
@@ -491,15 +514,10 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
     p->smem_bytes = f64 ? Ld::BYTES : Lf::BYTES;
     cudaError_t e = cudaSuccess;
     const int sb = (int)p->smem_bytes;
-    if (f64) {
-        e = cudaFuncSetAttribute(k_step_sym<double, MODE_STEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<double, MODE_DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<double, MODE_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-    } else {
-        e = cudaFuncSetAttribute(k_step_sym<float, MODE_STEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<float, MODE_DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_sym<float, MODE_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
-    }
+    const bool per = g.per[0] || g.per[1] || g.per[2];
+    const void* fn[3];
+    for (int m = 0; m < 3; ++m) fn[m] = f64 ? (const void*)sym_kernel<double>(m, per) : (const void*)sym_kernel<float>(m, per);
+    for (int m = 0; m < 3 && e == cudaSuccess; ++m) e = cudaFuncSetAttribute(fn[m], cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
     if (e != cudaSuccess) {
         *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
         return false;
@@ -514,23 +532,8 @@ inline bool sym_bind_stage(StreamPlan* p, void* xs)
 {
     const int bw = p->f64 ? SymLayout<double>::BW : SymLayout<float>::BW;
     if (!encode_map(&p->map_xi[2], p->f64, xs, p->g, bw, SymLayout<double>::TY + 4)) return false;
-    p->xi[2] = xs;
+    p->xi[2] = node_base(xs, p->g, p->f64);
     return true;
-}
-
-template <typename T>
-inline StreamArgs<T> sym_args(const StreamPlan& p, T dtg, int* flag)
-{
-    StreamArgs<T> a;
-    a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
-    a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
-    for (int c = 0; c < 3; ++c) a.twoh[c] = (T)p.g.twoh[c];
-    a.dtg = dtg;
-    a.tiles_x = p.tiles_x;
-    a.ntiles = p.tiles_x * p.tiles_y;
-    a.chunk_len = p.chunk_len;
-    a.flag = flag;
-    return a;
 }
 
 // One step (rhs = false: out = xi + dtg J x B) or one right-hand side (rhs = true: out = dtg J x B, dtg = gamma) of the
@@ -538,14 +541,10 @@ inline StreamArgs<T> sym_args(const StreamPlan& p, T dtg, int* flag)
 template <typename T>
 inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream, bool rhs = false, void* out = nullptr)
 {
-    const StreamArgs<T> a = sym_args<T>(p, dtg, flag);
+    const StreamArgs<T> a = stream_args<T>(p, dtg, flag);
     T* o = static_cast<T*>(out ? out : p.xi[1 - cur]);
-    if (rhs)
-        k_step_sym<T, MODE_RHS><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
-            p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), o, a);
-    else
-        k_step_sym<T, MODE_STEP><<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
-            p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), o, a);
+    sym_kernel<T>(rhs ? MODE_RHS : MODE_STEP, a.per != 0)<<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+        p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), o, a);
     return cudaGetLastError();
 }
 
@@ -553,9 +552,9 @@ inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* fla
 template <typename T>
 inline cudaError_t launch_sym_diag(const StreamPlan& p, int cur, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
 {
-    const StreamArgs<T> a = sym_args<T>(p, (T)0, flag);
+    const StreamArgs<T> a = stream_args<T>(p, (T)0, flag);
     *nblocks = a.ntiles * p.nchunks;
-    k_step_sym<T, MODE_DIAG><<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+    sym_kernel<T>(MODE_DIAG, a.per != 0)<<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
         p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();
 }

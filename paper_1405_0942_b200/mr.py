@@ -63,6 +63,10 @@ lib.mr_destroy.argtypes = [_ctx_p]
 lib.mr_destroy.restype = C.c_int
 lib.mr_adaptive_workspace_bytes.argtypes = [C.POINTER(mr_grid), C.c_int]
 lib.mr_adaptive_workspace_bytes.restype = C.c_size_t
+lib.mr_workspace_bytes_bc.argtypes = [C.POINTER(mr_grid), C.c_int, C.POINTER(C.c_int32)]
+lib.mr_workspace_bytes_bc.restype = C.c_size_t
+lib.mr_adaptive_workspace_bytes_bc.argtypes = [C.POINTER(mr_grid), C.c_int, C.POINTER(C.c_int32)]
+lib.mr_adaptive_workspace_bytes_bc.restype = C.c_size_t
 lib.mr_bind_adaptive_workspace.argtypes = [_ctx_p, C.c_void_p, C.c_size_t]
 lib.mr_bind_adaptive_workspace.restype = C.c_int
 lib.mr_step_adaptive.argtypes = [_ctx_p, C.c_double, C.c_double, C.POINTER(C.c_double), C.c_int, C.c_int64, C.POINTER(mr_adapt_stats),
@@ -111,9 +115,10 @@ def _raise(status, ctx):
     raise (NumericError if status == MR_ERR_NUMERIC else MrError)(status, msg)
 
 
-def workspace_bytes(n, dtype="f64") -> int:
+def workspace_bytes(n, dtype="f64", bc=("line_tied",) * 3) -> int:
     g = mr_grid(*[int(v) for v in n])
-    return int(lib.mr_workspace_bytes(C.byref(g), MR_F64 if dtype == "f64" else MR_F32))
+    bcs = (C.c_int32 * 3)(*[BOUNDARIES[b] for b in bc])
+    return int(lib.mr_workspace_bytes_bc(C.byref(g), MR_F64 if dtype == "f64" else MR_F32, bcs))
 
 
 def _op(op):
@@ -144,7 +149,8 @@ class Relaxation:
         if self.device.index is None:
             self.device = torch.device("cuda", torch.cuda.current_device())
         self._ctx = _ctx_p()
-        nbytes = workspace_bytes(self.n, dtype)
+        self.bc = tuple(bc)
+        nbytes = workspace_bytes(self.n, dtype, self.bc)
         if nbytes == 0:
             raise MrError(MR_ERR_INVALID_ARG, "invalid grid %r / dtype %r" % (self.n, dtype))
         with torch.cuda.device(self.device):
@@ -262,7 +268,8 @@ class Relaxation:
         with torch.cuda.device(self.device):
             if self._aworkspace is None:
                 g = mr_grid(*self.n)
-                nb = int(lib.mr_adaptive_workspace_bytes(C.byref(g), MR_F64 if self.dtype == "f64" else MR_F32))
+                bcs = (C.c_int32 * 3)(*[BOUNDARIES[b] for b in self.bc])
+                nb = int(lib.mr_adaptive_workspace_bytes_bc(C.byref(g), MR_F64 if self.dtype == "f64" else MR_F32, bcs))
                 with torch.cuda.stream(self.stream):
                     self._aworkspace = torch.empty(nb, dtype=torch.uint8, device=self.device)
                 self._check(lib.mr_bind_adaptive_workspace(self._ctx, self._aworkspace.data_ptr(), nb))

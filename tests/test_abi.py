@@ -45,6 +45,15 @@ def test_workspace_bytes_is_pure_host_arithmetic(mr):
     assert 2 * field <= b32 < 2 * field + (1 << 20)
     # odd sizes are padded to 16-element rows
     assert mr.workspace_bytes((17, 9, 7)) >= (3 * 3 * 32 * 9 * 7 + 3 * 17 * 9 * 7) * 8
+    # a periodic axis adds its ghost layers (two planes / rows, 16 bytes of columns either side) to the three padded fields
+    assert mr.workspace_bytes(n, "f64", ("line_tied",) * 3) == b64 == mr.lib.mr_workspace_bytes(C.byref(mr.mr_grid(*n)), mr.MR_F64)
+    bz = mr.workspace_bytes(n, "f64", ("line_tied", "line_tied", "periodic"))
+    assert bz - b64 == 3 * (3 * 256 * 256 * 4 * 8)
+    ball = mr.workspace_bytes(n, "f64", ("periodic",) * 3)
+    assert ball - b64 == 3 * 3 * 8 * (272 * 260 * 516 - 256 * 256 * 512)
+    bad = (C.c_int32 * 3)(0, 7, 0)
+    assert mr.lib.mr_workspace_bytes_bc(C.byref(mr.mr_grid(*n)), mr.MR_F64, bad) == 0
+    assert mr.lib.mr_adaptive_workspace_bytes_bc(C.byref(mr.mr_grid(*n)), mr.MR_F64, bad) == 0
 
 
 def _create(mr, n=(16, 16, 32), lo=(-4, -4, -8), hi=(4, 4, 8), bc=(0, 0, 0), gamma=1.0, dtype=0, ws=256, ws_bytes=1 << 40):

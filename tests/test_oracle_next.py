@@ -73,6 +73,14 @@ def test_step_control_follows_the_paper():
     assert ok and dtn == pytest.approx(0.5)
     ok, dtn = mro.step_control(0.1, 1e-30, lam0)
     assert ok and dtn == pytest.approx(0.5)
+    # reading Q22: just above Lambda0 the factor of Eq. 2.11 rounds to 1 (the value met on the IsoHelix run: the same trial
+    # would repeat for ever); a retry is at most 0.9 dt
+    ok, dtn = mro.step_control(0.3667726365104183, 1.0000000000000002e-08, 1e-8)
+    assert not ok and dtn == 0.9 * 0.3667726365104183
+    ok, dtn = mro.step_control(0.1, 1.2e-6, lam0)
+    assert not ok and dtn == pytest.approx(0.09, rel=1e-14)          # 1.2^-0.2 = 0.964 > 0.9
+    ok, dtn = mro.step_control(0.1, 2e-6, lam0)
+    assert not ok and dtn == pytest.approx(0.1 * 0.5 ** 0.2, rel=1e-14)   # 0.871 < 0.9: Eq. 2.11 as printed
 
 
 def test_adaptive_relaxation_on_config1():
