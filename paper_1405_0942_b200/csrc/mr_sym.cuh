@@ -114,9 +114,9 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int zface_lo = perz ? INT_MIN : 0, zface_hi = perz ? INT_MIN : nz - 1;    // the planes of the line-tied z faces
     const int zx_lo = perz ? -2 : 0, zx_hi = perz ? nz + 1 : nz - 1;               // the xi / b planes that exist
     const int k0 = chunk * a.chunk_len, k1 = min(k0 + a.chunk_len, nz);
-    const int kend = min(k1, zx_hi - (perz ? 1 : 0)); // planes k0 .. kend-1 are finished here (line-tied: nz-1 carried through)
-    const int first_p = max(k0 - 1, zx_lo + (perz ? 1 : 0));   // B is formed on the planes first_p .. kend
-    const int plast = min(kend + 1, zx_hi);         // last xi / b plane this item touches
+    const int kend = PER ? min(k1, zx_hi - (perz ? 1 : 0)) : min(k1, nz - 1);   // planes k0 .. kend-1 are finished here (line-tied: nz-1 carried through)
+    const int first_p = PER ? max(k0 - 1, zx_lo + (perz ? 1 : 0)) : max(k0 - 1, 0);   // B is formed on the planes first_p .. kend
+    const int plast = PER ? min(kend + 1, zx_hi) : min(kend + 1, nz - 1);           // last xi / b plane this item touches
     const V twoh[3] = { LN::bc(a.twoh[0]), LN::bc(a.twoh[1]), LN::bc(a.twoh[2]) };
 
     const bool pwarp = warp == NW - 1, producer = pwarp && lane == 0;
@@ -181,13 +181,20 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 #pragma unroll
     for (int e = 0; e < NV; ++e) {
         const int g = gi + e;
-        const bool real = has_node && row_real && g >= 0 && g < a.nx;
-        dom[e] = has_node && row_in && g >= -ox && g < a.nx + ox;
-        in_xy[e] = real && (perx || (g > 0 && g < a.nx - 1)) && (pery || (gj > 0 && gj < a.ny - 1));
-        st[e] = tilew && real;
+        if constexpr (PER) {
+            const bool real = has_node && row_real && g >= 0 && g < a.nx;
+            dom[e] = has_node && row_in && g >= -ox && g < a.nx + ox;
+            in_xy[e] = real && (perx || (g > 0 && g < a.nx - 1)) && (pery || (gj > 0 && gj < a.ny - 1));
+            st[e] = tilew && real;
+            if (real) edge |= ((g == 0 && !perx ? 1u : 0u) | (g == a.nx - 1 && !perx ? 2u : 0u) | (gj == 0 && !pery ? 4u : 0u) |
+                               (gj == a.ny - 1 && !pery ? 8u : 0u)) << (8 * e);
+        } else {
+            dom[e] = has_node && row_real && g >= 0 && g < a.nx;
+            in_xy[e] = g > 0 && g < a.nx - 1 && gj > 0 && gj < a.ny - 1;
+            st[e] = tilew && dom[e];
+            if (dom[e]) edge |= ((g == 0 ? 1u : 0u) | (g == a.nx - 1 ? 2u : 0u) | (gj == 0 ? 4u : 0u) | (gj == a.ny - 1 ? 8u : 0u)) << (8 * e);
+        }
         any_st = any_st || st[e];
-        if (real) edge |= ((g == 0 && !perx ? 1u : 0u) | (g == a.nx - 1 && !perx ? 2u : 0u) | (gj == 0 && !pery ? 4u : 0u) |
-                           (gj == a.ny - 1 && !pery ? 8u : 0u)) << (8 * e);
     }
 
     bool ok = true;
@@ -206,7 +213,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             xh[0][c] = LN::bc(T(0));
-            xh[1][c] = first_p > zx_lo ? from_global(in + c * a.comp, o) : LN::bc(T(0)); // phase 0 reads xi(first_p - 1) from xh[1]
+            xh[1][c] = (PER ? first_p > zx_lo : first_p > 0) ? from_global(in + c * a.comp, o) : LN::bc(T(0)); // phase 0 reads xi(first_p - 1) from xh[1]
 #pragma unroll
             for (int q = 0; q < 4; ++q) Bh[q][c] = LN::bc(T(0));
         }
@@ -252,7 +259,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     if (!pwarp) {        // the planes first_p, first_p + 1 and, for the one-sided difference on the bottom face, 2
         ptx::mbar_wait(bar + 8u, 0u);
         ptx::mbar_wait(bar + 16u, 0u);
-        if (first_p == zface_lo) ptx::mbar_wait(bar + 24u, 0u);
+        if (PER ? first_p == zface_lo : first_p == 0) ptx::mbar_wait(bar + 24u, 0u);
     }
     int p = first_p;
     uint32_t gpar = 0u;                                      // parity of the group of four planes
@@ -279,7 +286,8 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
                 dF[c][2] = LN::ld(f2p + c * CSX) - xp[c];
                 bq[c] = LN::ld(pb + S0 * L::SLOTB + c * CSB);
             }
-            const unsigned special = edge | (p == zface_lo ? 16u : 0u) | (p == zface_hi ? 32u : 0u);
+            const unsigned special = PER ? (edge | (p == zface_lo ? 16u : 0u) | (p == zface_hi ? 32u : 0u))
+                                         : (edge | (p == 0 ? 16u : 0u) | (p == nz - 1 ? 32u : 0u));
             if (special) {
                 if (special & 16u) {            // bottom face: -3 x(0) + 4 x(1) - x(2)
                     const T* f3 = px + S2 * L::SLOTX;
@@ -326,7 +334,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             LN::st(d + 2 * BCS, Bp[2]);
             if constexpr (TILE) {
                 V sn = LN::bc(a.dtg) * inv;
-                const bool kin = p != zface_lo && p != zface_hi;
+                const bool kin = PER ? (p != zface_lo && p != zface_hi) : (p > 0 && p < nz - 1);
 #pragma unroll
                 for (int e = 0; e < NV; ++e)
                     if (!(kin && in_xy[e])) LN::set(sn, e, T(0));
