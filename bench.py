@@ -270,6 +270,8 @@ def run_ours(args):
     sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype, device="cuda:%d" % local_rank)
     if args.variant != "auto":
         sim.set_variant(args.variant)
+    if args.no_graphs:
+        sim.set_variant("nograph")
     sim.set_B0(torch.from_numpy(B0).to("cuda", dtype=td))
 
     def reset_state():
@@ -448,6 +450,7 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-regimes", action="store_true", help="skip the burst / sustained records")
+    ap.add_argument("--no-graphs", action="store_true", help="mr_step launches every step itself (small grids replay CUDA graphs by default)")
     args = ap.parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)

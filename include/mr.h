@@ -186,8 +186,10 @@ int64_t mr_launch_count(const mr_ctx* ctx);
 const char* mr_step_variant(const mr_ctx* ctx);
 
 /* Choose the step kernel.  "auto" (default): the streaming TMA kernels (mimetic: csrc/mr_sym.cuh, direct:
- * csrc/mr_direct.cuh) when every axis is line-tied.  "generic": the global-memory kernels of csrc/mr_generic.cuh for both operators (one thread per
- * node, every stencil value straight from global memory): the A/B reference of the tests.  Both agree to rounding. */
+ * csrc/mr_direct.cuh).  "generic": the global-memory kernels of csrc/mr_generic.cuh for both operators (one thread per
+ * node, every stencil value straight from global memory): the A/B reference of the tests.  Both agree to rounding.
+ * "graph" (default) / "nograph": whether mr_step, on a grid whose fields fit the L2 (launch-latency bound), replays its
+ * launches sixteen steps at a time as a CUDA graph; the kernels and the results are the same either way. */
 mr_status mr_set_variant(mr_ctx* ctx, const char* name);
 
 #ifdef __cplusplus

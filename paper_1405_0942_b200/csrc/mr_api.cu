@@ -93,7 +93,21 @@ struct mr_ctx {
     bool plans_built;
     StreamPlan plan_dir;   // the streaming kernel of the direct-derivative operator (mr_direct.cuh)
     StreamPlan plan_mim;   // the streaming kernel of the mimetic operator (mr_sym.cuh)
+    // mr_step on a grid that lives in the L2: kStepsPerGraph steps captured once as a CUDA graph and replayed (the step is
+    // bound by launch latency there); the key is everything a captured launch depends on
+    cudaGraphExec_t step_graph = nullptr;
+    cudaStream_t cap_stream = nullptr;     // the capture is recorded on a stream of the library's own (the caller's may be the
+                                           // legacy default stream, which cannot be captured); the graph runs on the caller's
+    int sg_op = -1, sg_cur = -1, sg_variant = -1;
+    double sg_dtg = 0.0;
+    bool graphs_enabled = true;
     std::string err;
+
+    ~mr_ctx()
+    {
+        if (step_graph) cudaGraphExecDestroy(step_graph);
+        if (cap_stream) cudaStreamDestroy(cap_stream);
+    }
 
     // a padded field starts at *_raw (what the tensor maps and the elementwise kernels span); the kernels that index by
     // node get the address of the node (0, 0, 0)
@@ -299,15 +313,77 @@ mr_status launch_pass(mr_ctx* c, mr_operator op, int in, void* out, double dtg_d
     return MR_OK;
 }
 
+constexpr int kStepsPerGraph = 16;          // even: the state is back in the buffer it started from
+
+template <typename T>
+mr_status launch_steps(mr_ctx* c, int64_t n, double dtg, mr_operator op)
+{
+    for (int64_t s = 0; s < n; ++s) {
+        mr_status st = launch_pass<T>(c, op, c->cur, c->xi(1 - c->cur), dtg, false);
+        if (st != MR_OK) return st;
+        wrap_ghosts<T>(c, c->xi(1 - c->cur));
+        c->cur = 1 - c->cur;
+    }
+    return MR_OK;
+}
+
+// the graph of kStepsPerGraph steps from the buffer c->cur with this operator, dt and kernel choice (captured on first use,
+// re-captured when any of them changes); null if the stream cannot be captured right now (e.g. the caller is capturing)
+template <typename T>
+cudaGraphExec_t step_graph_for(mr_ctx* c, double dtg, mr_operator op)
+{
+    if (c->step_graph && c->sg_op == (int)op && c->sg_cur == c->cur && c->sg_variant == c->force_variant && c->sg_dtg == dtg)
+        return c->step_graph;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(c->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return nullptr; }
+    if (c->step_graph) { cudaGraphExecDestroy(c->step_graph); c->step_graph = nullptr; }
+    ensure_plans(c);                                   // (tensor maps and function attributes: not inside a capture)
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        c->cap_stream = nullptr;
+        cudaGetLastError();
+        return nullptr;
+    }
+    if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    const int64_t launches0 = c->launches;
+    const int cur0 = c->cur;
+    cudaStream_t user = c->stream;
+    c->stream = c->cap_stream;
+    const mr_status st = launch_steps<T>(c, kStepsPerGraph, dtg, op);
+    c->stream = user;
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+    c->launches = launches0;                            // nothing ran
+    c->cur = cur0;
+    if (st != MR_OK || e != cudaSuccess || !g) { if (g) cudaGraphDestroy(g); cudaGetLastError(); return nullptr; }
+    cudaGraphExec_t ex = nullptr;
+    if (cudaGraphInstantiate(&ex, g, 0) != cudaSuccess) { ex = nullptr; cudaGetLastError(); }
+    cudaGraphDestroy(g);
+    c->step_graph = ex;
+    c->sg_op = (int)op; c->sg_cur = c->cur; c->sg_variant = c->force_variant; c->sg_dtg = dtg;
+    return ex;
+}
+
 template <typename T>
 mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
 {
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
-    for (int64_t s = 0; s < n; ++s) {
-        mr_status st = launch_pass<T>(c, op, c->cur, c->xi(1 - c->cur), dt * c->gamma, false);
+    const double dtg = dt * c->gamma;
+    int64_t left = n;
+    // a grid whose three fields fit the L2 is bound by launch latency: replay kStepsPerGraph steps per graph launch
+    if (c->graphs_enabled && n >= 2 * kStepsPerGraph && 3 * c->L.field_bytes <= ((size_t)96 << 20)) {
+        if (cudaGraphExec_t ex = step_graph_for<T>(c, dtg, op)) {
+            const int64_t per_graph = (c->any_periodic ? 2 : 1) * kStepsPerGraph;
+            for (; left >= kStepsPerGraph; left -= kStepsPerGraph) {
+                MR_CUDA(c, cudaGraphLaunch(ex, c->stream));
+                c->launches += per_graph;
+            }
+            c->variant = streaming(c, op) ? (op == MR_OP_MIMETIC ? c->plan_mim.name : c->plan_dir.name)
+                                          : (op == MR_OP_MIMETIC ? "generic_mimetic" : "generic_direct");
+        }
+    }
+    {
+        mr_status st = launch_steps<T>(c, left, dtg, op);
         if (st != MR_OK) return st;
-        wrap_ghosts<T>(c, c->xi(1 - c->cur));
-        c->cur = 1 - c->cur;
     }
     MR_CUDA(c, cudaGetLastError());
     c->time += dt * (double)n;
@@ -838,6 +914,8 @@ extern "C" mr_status mr_set_variant(mr_ctx* ctx, const char* name)
     if (!ctx || !name) return MR_ERR_INVALID_ARG;
     if (!std::strcmp(name, "auto")) ctx->force_variant = 0;
     else if (!std::strcmp(name, "generic")) ctx->force_variant = 1;
-    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto or generic");
+    else if (!std::strcmp(name, "graph")) ctx->graphs_enabled = true;        // (the default) mr_step replays CUDA graphs on small grids
+    else if (!std::strcmp(name, "nograph")) ctx->graphs_enabled = false;
+    else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto, generic, graph or nograph");
     return MR_OK;
 }

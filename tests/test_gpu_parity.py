@@ -261,6 +261,32 @@ def test_zero_steps_is_a_no_op(mr):
     assert np.array_equal(sim.get_fields(x=True)["x"].cpu().numpy(), x0)
 
 
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+@pytest.mark.parametrize("name,bc", [("C1", None), ("ragged", None), ("C1", ("line_tied", "line_tied", "periodic"))])
+def test_graph_replay_is_bit_identical_to_plain_launches(mr, op, name, bc):
+    """on an L2-resident grid mr_step replays sixteen captured steps per CUDA-graph launch.  Same kernels, same
+    order: the state after 37 + 64 + 3 steps (graph launches, a remainder, a re-capture from the other buffer, a call too
+    short for a graph) equals the one from plain launches bit for bit, and the launch counter counts the same launches."""
+    g, x0, B0, dt = case(name)
+    bc = bc or ("line_tied",) * 3
+    if bc[2] == "periodic":
+        x0 = I.reference_grid(g)                    # (the C1 field is not periodic in z: start undisplaced, step little)
+    sims = {}
+    for v in ("graph", "nograph"):
+        sim = make_sim(mr, g, x0, B0, bc=bc)
+        sim.set_variant(v)
+        l0 = sim.launch_count
+        for n in (37, 64, 3):
+            sim.step(n, dt, op)
+        launches = sim.launch_count - l0
+        sims[v] = (sim.get_xi().cpu().numpy(), launches, sim.diagnostics(op))
+    assert np.array_equal(sims["graph"][0], sims["nograph"][0])
+    assert sims["graph"][1] == sims["nograph"][1] == 104 * (2 if bc[2] == "periodic" else 1)
+    assert sims["graph"][2]["steps"] == 104 and sims["graph"][2]["energy"] == sims["nograph"][2]["energy"]
+    with pytest.raises(mr.MrError):
+        sim.set_variant("no-such-kernel")
+
+
 def test_full_size_config4_one_step_matches_oracle(mr):
     """BASELINE configs[3] at full size (256x256x512, the bench workload and launch configuration), initial grid
     smoothly displaced so that every term is exercised: x after one step and the diagnostics against the oracle
