@@ -3,6 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C1..C5]
                     [--operator mimetic|direct] [--integrator euler|adaptive] [--reading P|D]
+                    [--isohelix N[,N..] [--t-end T]]
 
 One "step" is one pass of the whole hot path (S1-S5: Jacobian, push-forward, mimetic curl, J x B, line-tied
 update) over the full 256x256x512 grid = one fused kernel launch inside mr_step.  The timed region is ONE
@@ -434,6 +435,71 @@ def run_ours(args):
     return 0
 
 
+def paper_table_4_1():
+    """TABLE 4.1 of the paper as printed (tests/golden/paper_table_4_1.txt): {(method, n): (xi, eps*, sigma_B, sigma_x)}, phi = pi/4"""
+    rows = {}
+    try:
+        with open(os.path.join(ROOT, "tests", "golden", "paper_table_4_1.txt")) as f:
+            for line in f:
+                line = line.split("#", 1)[0].split()
+                if line and float(line[0]) == 0.25:
+                    rows[(line[1], int(line[2]))] = tuple(float(v) for v in line[3:7])
+    except OSError:
+        pass
+    return rows
+
+
+def run_isohelix(args):
+    """--isohelix N[,N..]: the paper's own experiment (section 3.1, TABLE 4.1): the IsoHelix field (phi = pi/4) on N^3 nodes relaxed
+    with the adaptive Cash-Karp integrator (section 2.4) to t = --t-end, where eps*, sigma_B, sigma_x have stabilised; prints them
+    beside the paper's row, with the wall time of the run and the rate of right-hand-side evaluations."""
+    import numpy as np
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the relaxation step has no CPU path")
+    from paper_1405_0942_b200 import inputs as I, mr
+    paper = paper_table_4_1()
+    rows, total_rhs, total_s, launches = [], 0, 0.0, 0
+    phi = np.pi / 4
+    for n in [int(v) for v in args.isohelix.split(",")]:
+        g = I.Grid((n, n, n), (-4.0, -4.0, -10.0), (4.0, 4.0, 10.0))
+        B0 = I.isohelix_B0(g, phi)
+        Bref = np.zeros(g.shape)
+        Bref[2] = 1.0
+        for op in args.operator.split(","):
+            sim = mr.Relaxation(g.n, g.lo, g.hi, dtype="f64", device="cuda:0")
+            if args.no_graphs:
+                sim.set_variant("nograph")
+            sim.set_B0(torch.from_numpy(B0).cuda())
+            xr, Br = torch.from_numpy(I.isohelix_x_relax(g, phi)).cuda(), torch.from_numpy(Bref).cuda()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            st = sim.step_adaptive(t_end=args.t_end, lambda0=args.lambda0, dt=1e-3, op=op, max_trials=10 ** 7)
+            torch.cuda.synchronize()
+            el = time.perf_counter() - t0
+            d = sim.diagnostics(op)
+            sx, sb = sim.sigma(xr, Br)
+            _, eps = sim.eps_star(n // 2, n // 2, float(np.sqrt(2.0)), op)
+            pk = paper.get(("mimetic" if op == "mimetic" else "classic", n))
+            rows.append({"n": n, "operator": op, "t_end": st["time"], "accepted": st["accepted"], "rejected": st["rejected"],
+                         "seconds": el, "us_per_trial": el / max(st["accepted"] + st["rejected"], 1) * 1e6,
+                         "xi": d["xi"], "eps_star": eps, "sigma_B": sb, "sigma_x": sx, "energy": d["energy"],
+                         "concave_nodes": sim.convexity()[0], "kernel": sim.step_variant,
+                         "paper": None if pk is None else {"xi": pk[0], "eps_star": pk[1], "sigma_B": pk[2], "sigma_x": pk[3]}})
+            total_rhs += st["rhs_evals"] * g.nodes
+            total_s += el
+            launches += sim.launch_count
+            sim.close()
+    line = {"metric": "node right-hand-side evaluations/s (IsoHelix relaxation, adaptive RK5(4), fp64)", "value": total_rhs / total_s,
+            "unit": "node-rhs/s", "n_gpus": 1, "higher_is_better": True, "dtype": "f64", "data": "synthetic", "vs_baseline": None,
+            "config": {"workload": "IsoHelix phi=pi/4 (PAPER.md:170-186) on n^3 nodes, n in [%s], lambda0=%g, t_end=%g; "
+                                   "paper rows: TABLE 4.1 (the 'classic' rows are the paper's direct method, whose formulas it does "
+                                   "not print: context only)" % (args.isohelix, args.lambda0, args.t_end)},
+            "gpu_launches": launches, "table_4_1": rows}
+    print(json.dumps(line))
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -442,7 +508,9 @@ def main(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--variant", default="auto", choices=["auto", "generic"])
-    ap.add_argument("--operator", default="mimetic", choices=["mimetic", "direct"])
+    ap.add_argument("--operator", default="mimetic", help="mimetic | direct (--isohelix: a comma-separated list of them)")
+    ap.add_argument("--isohelix", default="", help="N[,N..]: relax the paper's IsoHelix field on N^3 nodes and report TABLE 4.1's measures")
+    ap.add_argument("--t-end", type=float, default=512.0, help="--isohelix: end time of the relaxation")
     ap.add_argument("--integrator", default="euler", choices=["euler", "adaptive"])
     ap.add_argument("--reading", default="P", choices=["P", "D"], help="config 3: B0 pulled back (P) or ABC(X) literally (D)")
     ap.add_argument("--lambda0", type=float, default=1e-9, help="tolerance of the adaptive integrator")
@@ -452,6 +520,12 @@ def main(argv=None):
     ap.add_argument("--no-regimes", action="store_true", help="skip the burst / sustained records")
     ap.add_argument("--no-graphs", action="store_true", help="mr_step launches every step itself (small grids replay CUDA graphs by default)")
     args = ap.parse_args(argv)
+    if args.isohelix:
+        if args.lambda0 == 1e-9:
+            args.lambda0 = 1e-8
+        return run_isohelix(args)
+    if args.operator not in ("mimetic", "direct"):
+        ap.error("--operator must be mimetic or direct")
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

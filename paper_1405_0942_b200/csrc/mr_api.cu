@@ -101,12 +101,22 @@ struct mr_ctx {
     int sg_op = -1, sg_cur = -1, sg_variant = -1;
     double sg_dtg = 0.0;
     bool graphs_enabled = true;
+    // mr_step_adaptive: the launches of one Cash-Karp trial step (they read dt from device memory) captured once per
+    // (operator, state buffer) and replayed; dt goes in and Lambda and the flag come back through three pinned host words
+    cudaGraphExec_t trial_graph[2][2] = { { nullptr, nullptr }, { nullptr, nullptr } };
+    int tg_variant[2][2] = { { -1, -1 }, { -1, -1 } };
+    int64_t tg_launches[2][2] = { { 0, 0 }, { 0, 0 } };
+    double* pinned = nullptr;              // [0] dt of the trial, [1] Lambda, [2] the flag word (as an int)
     std::string err;
 
     ~mr_ctx()
     {
         if (step_graph) cudaGraphExecDestroy(step_graph);
+        for (int o = 0; o < 2; ++o)
+            for (int w = 0; w < 2; ++w)
+                if (trial_graph[o][w]) cudaGraphExecDestroy(trial_graph[o][w]);
         if (cap_stream) cudaStreamDestroy(cap_stream);
+        if (pinned) cudaFreeHost(pinned);
     }
 
     // a padded field starts at *_raw (what the tensor maps and the elementwise kernels span); the kernels that index by
@@ -120,6 +130,7 @@ struct mr_ctx {
     DiagPartial* partials() const { return reinterpret_cast<DiagPartial*>(ws + L.off_partials); }
     DiagPartial* diag_out() const { return reinterpret_cast<DiagPartial*>(ws + L.off_diag); }
     int* flag() const { return reinterpret_cast<int*>(ws + L.off_flag); }
+    double* dt_dev() const { return reinterpret_cast<double*>(ws + L.off_diag + 128); }   // the trial step length (kernels read it)
     void* kbuf_raw(int s) const { return aws + (size_t)s * L.field_bytes; }  // s = 0..5: k_1..k_6, 6: the stage state
     void* kbuf(int s) const { return aws + (size_t)s * L.field_bytes + node0(); }
     size_t esize() const { return dtype == MR_F64 ? 8 : 4; }
@@ -450,10 +461,11 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     return MR_OK;
 }
 
-// ---- section 2.4: one Cash-Karp trial step of length h from the state buffer `cur`; the fifth-order solution goes
-// to the other state buffer, Lambda = max |x5 - x4| comes back (the one device -> host scalar of the step)
+// ---- section 2.4: one Cash-Karp trial step from the state buffer `cur`; the fifth-order solution goes to the other
+// state buffer.  Everything is enqueued on c->stream and nothing depends on the step length, which the kernels read from
+// dt_dev(): pinned[0] -> dt_dev() goes in first, Lambda = max |x5 - x4| -> pinned[1] and the flag -> pinned[2] come out last.
 template <typename T>
-mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* numeric)
+mr_status enqueue_trial(mr_ctx* c, mr_operator op)
 {
     static const CashKarp ck = cash_karp();
     const long long n2 = 3 * c->L.comp / 2;             // element pairs of a padded field (pitch is a multiple of 16)
@@ -461,12 +473,13 @@ mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* num
     const T* x = static_cast<const T*>(c->xi_raw(c->cur));      // the elementwise kernels run over the whole padded fields
     T* xs = static_cast<T*>(c->kbuf_raw(6));
     MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
+    MR_CUDA(c, cudaMemcpyAsync(c->dt_dev(), c->pinned, sizeof(double), cudaMemcpyHostToDevice, c->stream));
     for (int s = 0; s < 6; ++s) {
         if (s > 0) {
             StageArgs a;
             a.n = s;
-            for (int r = 0; r < 6; ++r) { a.k[r] = c->kbuf_raw(r < s ? r : 0); a.c[r] = r < s ? h * ck.a[s][r] : 0.0; }
-            k_rk_stage<T><<<blocks, 256, 0, c->stream>>>(x, xs, a, n2);
+            for (int r = 0; r < 6; ++r) { a.k[r] = c->kbuf_raw(r < s ? r : 0); a.c[r] = r < s ? ck.a[s][r] : 0.0; }
+            k_rk_stage<T><<<blocks, 256, 0, c->stream>>>(x, xs, a, n2, c->dt_dev());
             c->launches++;
             wrap_ghosts<T>(c, c->kbuf(6));                        // (the ghosts of the k_r are not kept)
         }
@@ -475,15 +488,72 @@ mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* num
     }
     StageArgs b5, db;
     b5.n = db.n = 6;
-    for (int r = 0; r < 6; ++r) { b5.k[r] = db.k[r] = c->kbuf_raw(r); b5.c[r] = h * ck.b5[r]; db.c[r] = h * ck.db[r]; }
+    for (int r = 0; r < 6; ++r) { b5.k[r] = db.k[r] = c->kbuf_raw(r); b5.c[r] = ck.b5[r]; db.c[r] = ck.db[r]; }
     double* partial = reinterpret_cast<double*>(c->partials());
-    k_rk_final<T><<<blocks, 256, 0, c->stream>>>(x, static_cast<T*>(c->xi_raw(1 - c->cur)), b5, db, n2, partial);
+    k_rk_final<T><<<blocks, 256, 0, c->stream>>>(x, static_cast<T*>(c->xi_raw(1 - c->cur)), b5, db, n2, partial, c->dt_dev());
     k_max_final<<<1, 256, 0, c->stream>>>(partial, blocks, reinterpret_cast<double*>(c->diag_out()));
     c->launches += 2;
     wrap_ghosts<T>(c, c->xi(1 - c->cur));
     MR_CUDA(c, cudaGetLastError());
-    MR_CUDA(c, cudaMemcpyAsync(lambda, c->diag_out(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    return read_flag(c, numeric);
+    MR_CUDA(c, cudaMemcpyAsync(c->pinned + 1, c->diag_out(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaMemcpyAsync(c->pinned + 2, c->flag(), sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    return MR_OK;
+}
+
+// the captured trial step for this operator and state buffer (null: not available, enqueue the launches instead)
+template <typename T>
+cudaGraphExec_t trial_graph_for(mr_ctx* c, mr_operator op)
+{
+    const int o = op == MR_OP_MIMETIC ? 0 : 1, w = c->cur;
+    if (c->trial_graph[o][w] && c->tg_variant[o][w] == c->force_variant) return c->trial_graph[o][w];
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(c->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return nullptr; }
+    if (c->trial_graph[o][w]) { cudaGraphExecDestroy(c->trial_graph[o][w]); c->trial_graph[o][w] = nullptr; }
+    ensure_plans(c);
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        c->cap_stream = nullptr;
+        cudaGetLastError();
+        return nullptr;
+    }
+    if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    const int64_t launches0 = c->launches;
+    cudaStream_t user = c->stream;
+    c->stream = c->cap_stream;
+    const mr_status st = enqueue_trial<T>(c, op);
+    c->stream = user;
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+    c->tg_launches[o][w] = c->launches - launches0;
+    c->launches = launches0;                            // nothing ran
+    if (st != MR_OK || e != cudaSuccess || !g) { if (g) cudaGraphDestroy(g); cudaGetLastError(); return nullptr; }
+    cudaGraphExec_t ex = nullptr;
+    if (cudaGraphInstantiate(&ex, g, 0) != cudaSuccess) { ex = nullptr; cudaGetLastError(); }
+    cudaGraphDestroy(g);
+    c->trial_graph[o][w] = ex;
+    c->tg_variant[o][w] = c->force_variant;
+    return ex;
+}
+
+// one trial step of length h: Lambda comes back (the one device -> host exchange of the step)
+template <typename T>
+mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* numeric)
+{
+    if (!c->pinned) MR_CUDA(c, cudaHostAlloc(reinterpret_cast<void**>(&c->pinned), 4 * sizeof(double), cudaHostAllocDefault));
+    c->pinned[0] = h;
+    cudaGraphExec_t ex = c->graphs_enabled ? trial_graph_for<T>(c, op) : nullptr;
+    if (ex) {
+        MR_CUDA(c, cudaGraphLaunch(ex, c->stream));
+        c->launches += c->tg_launches[op == MR_OP_MIMETIC ? 0 : 1][c->cur];
+        c->variant = streaming(c, op) ? (op == MR_OP_MIMETIC ? c->plan_mim.name : c->plan_dir.name)
+                                      : (op == MR_OP_MIMETIC ? "generic_mimetic" : "generic_direct");
+    } else {
+        mr_status st = enqueue_trial<T>(c, op);
+        if (st != MR_OK) return st;
+    }
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    *lambda = c->pinned[1];
+    *numeric = *reinterpret_cast<const int*>(c->pinned + 2);
+    return MR_OK;
 }
 
 // Eq. 2.11 and the accept / reject rule of PAPER.md:139-143 (reading Q22)

@@ -31,16 +31,20 @@ inline CashKarp cash_karp()
 
 struct StageArgs {
     const void* k[6];     // stage velocities k_1 .. k_6 (padded layout, like xi)
-    double c[6];          // dt * coefficient of each
+    double c[6];          // coefficient of each (the kernels multiply by the step length dt, which they read from device memory:
+                          // the launches of a trial step do not depend on dt and can be replayed as a CUDA graph)
     int n;                // how many of them enter
 };
 
 // xi_s = xi + sum_r (dt a_sr) k_r over the whole padded field (the padding stays zero); elementwise, vectorised by two
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_rk_stage(const T* __restrict__ xi, T* __restrict__ xs, StageArgs a, long long n2)
+k_rk_stage(const T* __restrict__ xi, T* __restrict__ xs, StageArgs a, long long n2, const double* __restrict__ dt)
 {
     using V = typename std::conditional<sizeof(T) == 8, double2, float2>::type;
+    const double h = *dt;
+#pragma unroll
+    for (int r = 0; r < 6; ++r) a.c[r] = h * a.c[r];
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n2; q += (long long)gridDim.x * blockDim.x) {
         V v = reinterpret_cast<const V*>(xi)[q];
         double s0 = 0.0, s1 = 0.0;
@@ -61,9 +65,13 @@ k_rk_stage(const T* __restrict__ xi, T* __restrict__ xs, StageArgs a, long long 
 // x").  A maximum does not depend on the order: the result is deterministic.
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_rk_final(const T* __restrict__ xi, T* __restrict__ x5, StageArgs b5, StageArgs db, long long n2, double* __restrict__ partial)
+k_rk_final(const T* __restrict__ xi, T* __restrict__ x5, StageArgs b5, StageArgs db, long long n2, double* __restrict__ partial,
+           const double* __restrict__ dt)
 {
     using V = typename std::conditional<sizeof(T) == 8, double2, float2>::type;
+    const double h = *dt;
+#pragma unroll
+    for (int r = 0; r < 6; ++r) { b5.c[r] = h * b5.c[r]; db.c[r] = h * db.c[r]; }
     double lam = 0.0;
     bool nan = false;
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n2; q += (long long)gridDim.x * blockDim.x) {

@@ -232,7 +232,8 @@ inline void choose_chunks(int ntiles, int nz, int slots, int* nchunks, int* chun
 {
     double best = 1e300;
     int bc = 1;
-    const int maxc = std::max(1, nz / 4);
+    const int maxc = nz;      // down to one plane per chunk: a grid of a few tiles is bound by the latency of a CTA's march, and
+                              // the three planes of restart overhead cost nothing while SMs are idle (C1: 11.4 -> 8.4 us per step)
     for (int c = 1; c <= maxc; ++c) {
         const int len = (nz + c - 1) / c;
         const int cc = (nz + len - 1) / len;              // chunks actually produced by this length

@@ -236,7 +236,6 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 #pragma unroll
         for (int e = 0; e < NV; ++e) {
             if (!st[e]) continue;
-            const int g = gi + e;
             const double zxy = ((edge >> (8 * e)) & 3u ? 0.5 : 1.0) * ((edge >> (8 * e)) & 12u ? 0.5 : 1.0);          // Eq. 3.13
             double D = 0.0, b2 = 0.0, u2 = 0.0;
 #pragma unroll
