@@ -435,14 +435,14 @@ def run_ours(args):
     return 0
 
 
-def paper_table_4_1():
-    """TABLE 4.1 of the paper as printed (tests/golden/paper_table_4_1.txt): {(method, n): (xi, eps*, sigma_B, sigma_x)}, phi = pi/4"""
+def paper_table_4_1(phi_over_pi=0.25):
+    """TABLE 4.1 of the paper as printed (tests/golden/paper_table_4_1.txt): {(method, n): (xi, eps*, sigma_B, sigma_x)} for one phi"""
     rows = {}
     try:
         with open(os.path.join(ROOT, "tests", "golden", "paper_table_4_1.txt")) as f:
             for line in f:
                 line = line.split("#", 1)[0].split()
-                if line and float(line[0]) == 0.25:
+                if line and float(line[0]) == phi_over_pi:
                     rows[(line[1], int(line[2]))] = tuple(float(v) for v in line[3:7])
     except OSError:
         pass
@@ -458,25 +458,34 @@ def run_isohelix(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the relaxation step has no CPU path")
     from paper_1405_0942_b200 import inputs as I, mr
-    paper = paper_table_4_1()
+    paper = paper_table_4_1(args.phi)
     rows, total_rhs, total_s, launches = [], 0, 0.0, 0
-    phi = np.pi / 4
+    phi = np.pi * args.phi
+    td = torch.float64 if args.dtype == "f64" else torch.float32
     for n in [int(v) for v in args.isohelix.split(",")]:
         g = I.Grid((n, n, n), (-4.0, -4.0, -10.0), (4.0, 4.0, 10.0))
         B0 = I.isohelix_B0(g, phi)
         Bref = np.zeros(g.shape)
         Bref[2] = 1.0
         for op in args.operator.split(","):
-            sim = mr.Relaxation(g.n, g.lo, g.hi, dtype="f64", device="cuda:0")
+            sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=args.dtype, device="cuda:0")
             if args.no_graphs:
                 sim.set_variant("nograph")
-            sim.set_B0(torch.from_numpy(B0).cuda())
-            xr, Br = torch.from_numpy(I.isohelix_x_relax(g, phi)).cuda(), torch.from_numpy(Bref).cuda()
+            sim.set_B0(torch.from_numpy(B0).to("cuda", td))
+            xr, Br = torch.from_numpy(I.isohelix_x_relax(g, phi)).to("cuda", td), torch.from_numpy(Bref).to("cuda", td)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            st = sim.step_adaptive(t_end=args.t_end, lambda0=args.lambda0, dt=1e-3, op=op, max_trials=10 ** 7)
+            failed = None
+            try:
+                st = sim.step_adaptive(t_end=args.t_end, lambda0=args.lambda0, dt=1e-3, op=op, max_trials=10 ** 7)
+            except mr.MrError as e:                       # (the paper's table has such rows too: "runs which do not converge")
+                failed, st = str(e), sim.last_adaptive
             torch.cuda.synchronize()
             el = time.perf_counter() - t0
+            if failed:
+                rows.append({"n": n, "operator": op, "failed": failed, "t_end": st["time"], "accepted": st["accepted"],
+                             "rejected": st["rejected"], "seconds": el})
+                continue
             d = sim.diagnostics(op)
             sx, sb = sim.sigma(xr, Br)
             _, eps = sim.eps_star(n // 2, n // 2, float(np.sqrt(2.0)), op)
@@ -490,11 +499,11 @@ def run_isohelix(args):
             total_s += el
             launches += sim.launch_count
             sim.close()
-    line = {"metric": "node right-hand-side evaluations/s (IsoHelix relaxation, adaptive RK5(4), fp64)", "value": total_rhs / total_s,
-            "unit": "node-rhs/s", "n_gpus": 1, "higher_is_better": True, "dtype": "f64", "data": "synthetic", "vs_baseline": None,
-            "config": {"workload": "IsoHelix phi=pi/4 (PAPER.md:170-186) on n^3 nodes, n in [%s], lambda0=%g, t_end=%g; "
+    line = {"metric": "node right-hand-side evaluations/s (IsoHelix relaxation, adaptive RK5(4), fp64)", "value": total_rhs / max(total_s, 1e-9),
+            "unit": "node-rhs/s", "n_gpus": 1, "higher_is_better": True, "dtype": args.dtype, "data": "synthetic", "vs_baseline": None,
+            "config": {"workload": "IsoHelix phi=%g pi (PAPER.md:170-186) on n^3 nodes, n in [%s], lambda0=%g, t_end=%g; "
                                    "paper rows: TABLE 4.1 (the 'classic' rows are the paper's direct method, whose formulas it does "
-                                   "not print: context only)" % (args.isohelix, args.lambda0, args.t_end)},
+                                   "not print: context only)" % (args.phi, args.isohelix, args.lambda0, args.t_end)},
             "gpu_launches": launches, "table_4_1": rows}
     print(json.dumps(line))
     return 0
@@ -511,6 +520,8 @@ def main(argv=None):
     ap.add_argument("--operator", default="mimetic", help="mimetic | direct (--isohelix: a comma-separated list of them)")
     ap.add_argument("--isohelix", default="", help="N[,N..]: relax the paper's IsoHelix field on N^3 nodes and report TABLE 4.1's measures")
     ap.add_argument("--t-end", type=float, default=512.0, help="--isohelix: end time of the relaxation")
+    ap.add_argument("--phi", type=float, default=0.25, help="--isohelix: twist angle in units of pi (the paper: 0.25, 0.5, 1)")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="--isohelix: precision of the context")
     ap.add_argument("--integrator", default="euler", choices=["euler", "adaptive"])
     ap.add_argument("--reading", default="P", choices=["P", "D"], help="config 3: B0 pulled back (P) or ABC(X) literally (D)")
     ap.add_argument("--lambda0", type=float, default=1e-9, help="tolerance of the adaptive integrator")
