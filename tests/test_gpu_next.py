@@ -281,15 +281,15 @@ def _table_4_1(golden_dir):
     return rows
 
 
-def _isohelix_run(mr, n, op, t_end, lam0=1e-8):
+def _isohelix_run(mr, n, op, t_end, lam0=1e-8, phi=np.pi / 4, dtype="f64"):
     g = I.Grid((n, n, n), (-4.0, -4.0, -10.0), (4.0, 4.0, 10.0))
-    phi = np.pi / 4
     B0 = I.isohelix_B0(g, phi)
-    sim = make_sim(mr, g, I.reference_grid(g), B0)
+    sim = make_sim(mr, g, I.reference_grid(g), B0, dtype=dtype)
     st = sim.step_adaptive(t_end=t_end, lambda0=lam0, dt=1e-3, op=op, max_trials=400000)
     Bref = np.zeros(g.shape)
     Bref[2] = 1.0
-    sx, sb = sim.sigma(dev(I.isohelix_x_relax(g, phi)), dev(Bref))
+    td = torch.float64 if dtype == "f64" else torch.float32
+    sx, sb = sim.sigma(dev(I.isohelix_x_relax(g, phi), td), dev(Bref, td))
     _, eps = sim.eps_star(n // 2, n // 2, np.sqrt(2.0), op)
     return sim, st, eps, sb, sx
 
@@ -312,6 +312,25 @@ def test_isohelix_relaxation_reproduces_table_4_1_on_the_gpu(mr, golden_dir, n, 
     # the paper's qualitative finding: the direct operator's relaxed state is far worse in eps*
     _, _, eps_d, sb_d, _ = _isohelix_run(mr, n, "direct", 128.0)
     assert eps_d > 20 * eps and sb_d > 5 * sb
+
+
+@pytest.mark.parametrize("phi_pi,n,dtype,t_end,tol", [(0.5, 33, "f64", 512.0, 0.04), (0.5, 33, "f32", 512.0, 0.04), (1.0, 33, "f64", 256.0, 0.06)])
+def test_isohelix_other_twist_angles_of_table_4_1(mr, golden_dir, phi_pi, n, dtype, t_end, tol):
+    """The phi = pi/2 and phi = pi rows of TABLE 4.1 (the paper ran them in single precision; eps*, sigma_B, sigma_x are set by the
+    discretisation, not by the precision).  Measured on the B200 at 33^3:
+        phi = pi/2: eps* 6.084e-2, sigma_B 1.459e-3, sigma_x 7.095e-3 (fp64 and fp32 alike)   paper: 6.1e-2, 1.5e-3, 7.1e-3
+        phi = pi  : eps* 5.33e-1,  sigma_B 6.38e-3,  sigma_x 2.58e-2                          paper: 5.4e-1, 6.4e-3, 2.7e-2
+    (65^3, `bench.py --isohelix 65 --phi 0.5 | 1.0`: 2.37e-3, 3.38e-4, 5.78e-3 | 2.70e-2, 1.33e-3, 2.08e-2 against the paper's
+    2.3e-3, 3.4e-4, 5.9e-3 | 2.7e-2, 1.4e-3, 2.1e-2.)  At phi = pi the coarse grid has concave nodes."""
+    xi_p, eps_p, sB_p, sx_p = _table_4_1(golden_dir)[(phi_pi, "mimetic", n)]
+    sim, st, eps, sb, sx = _isohelix_run(mr, n, "mimetic", t_end, lam0=1e-8 if dtype == "f64" else 1e-6, phi=np.pi * phi_pi, dtype=dtype)
+    assert st["time"] == t_end
+    assert eps == pytest.approx(eps_p, rel=tol), eps
+    assert sb == pytest.approx(sB_p, rel=tol), sb
+    assert sx == pytest.approx(sx_p, rel=tol), sx
+    if dtype == "f32":                          # the paper's xi of this (single-precision) run: 3.0e-5; same order here
+        assert 0.2 * xi_p < sim.diagnostics()["xi"] < 5 * xi_p
+    assert (sim.convexity()[0] > 0) == (phi_pi == 1.0)
 
 
 def test_isohelix_relaxation_on_the_gpu_follows_the_oracle(mr):

@@ -71,6 +71,51 @@ def test_one_step_matches_oracle(mr, name, op, variant):
     assert np.array_equal(x1[m], np.asarray(x0)[m])
 
 
+@pytest.mark.parametrize("n", [(4096, 5, 5), (5, 4096, 5), (5, 5, 4096), (4096, 6, 7)])
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_maximum_extents_match_oracle(mr, n, op, dtype):
+    """The largest extent the ABI accepts (4096) along each axis with the smallest one (5) along the others: 128 tiles in x with
+    every node next to a face in y and z, 256 tiles in y, a march of 4096 planes cut into as many z-chunks as there are SMs.
+    Three steps and S6 against the oracle (fp32: against the oracle through the displacement, Q15)."""
+    lo = tuple(-0.01 * (m - 1) for m in n)
+    hi = tuple(0.01 * (m - 1) for m in n)                       # h = 0.02 on every axis
+    g = I.Grid(n, lo, hi)
+    X = I.reference_grid(g)
+    s = [2.0 * np.pi * (X[a] - lo[a]) / 0.64 for a in range(3)]                # wavelength 32 h
+    env = np.ones_like(X[0])
+    for a in range(3):
+        env = env * np.sin(np.pi * (X[a] - lo[a]) / (hi[a] - lo[a]))
+    env[0], env[-1], env[:, 0], env[:, -1], env[:, :, 0], env[:, :, -1] = 0.0, 0.0, 0.0, 0.0, 0.0, 0.0    # exactly zero on the faces
+    x0 = X.copy()
+    x0[0] += 0.004 * env * np.sin(s[1] + s[2])
+    x0[1] += 0.003 * env * np.cos(s[0]) * np.sin(s[2] + 0.3)
+    x0[2] += 0.004 * env * np.sin(s[0] + 0.5 * s[1])
+    B0 = np.empty_like(X)
+    B0[0] = 0.3 * np.sin(s[2]) + 0.1 * np.cos(s[1])
+    B0[1] = 0.2 * np.cos(s[0] + s[2])
+    B0[2] = 1.0 + 0.2 * np.sin(s[0]) * np.cos(s[1])
+    dt = 0.5 * I.stable_dt(B0, g)
+    sim = make_sim(mr, g, x0, B0, dtype=dtype)
+    d = sim.diagnostics(op)
+    sim.step(3, dt, op)
+    assert sim.step_variant.startswith("sym" if op == "mimetic" else "direct_tma")
+    o = mro.diagnostics(g.n, g.lo, g.hi, x0, B0, op=opcode(op))
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 3, op=opcode(op))
+    tol = TOL_STEP if dtype == "f64" else TOL_F32
+    for k in ("energy", "max_jxb", "min_det"):           # (an fp32 context forms J in fp32: eps |B| / 2h of it is rounding)
+        assert d[k] == pytest.approx(o[k], rel=10 * tol if (dtype == "f64" or k != "max_jxb") else 2e-3), k
+    xi = sim.get_xi().double().cpu().numpy()
+    assert np.abs(xi - (ref - X)).max() < 10 * tol * np.abs(ref - X).max()
+    moved = np.abs(ref - x0).max()
+    assert moved > 0
+    if dtype == "f64":
+        assert np.abs(xi - (ref - X)).max() < 1e-9 * moved
+    m = np.ones(xi.shape, bool)
+    m[:, 1:-1, 1:-1, 1:-1] = False
+    assert not xi[m].any()                                      # line-tied faces: the displacement stays exactly zero
+
+
 @pytest.mark.parametrize("name,steps", [("C1", 100), ("C2_small", 100), ("C3_small", 100), ("ragged", 100)])
 @pytest.mark.parametrize("variant", ["auto", "generic"])
 def test_100_steps_match_oracle(mr, name, steps, variant):
