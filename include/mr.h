@@ -16,8 +16,10 @@
  *   - "_dev" pointers are CUDA device pointers on the context's device; "_host" pointers are host pointers
  *     (pinned memory makes the copies asynchronous and fast, pageable memory also works).
  *   - Ownership: the CALLER owns every device and host buffer and the stream.  The library never allocates
- *     device memory: mr_create binds a caller-provided workspace of at least mr_workspace_bytes() bytes
- *     (256-byte aligned) that must outlive the context.  mr_ctx itself is host memory owned by the library.
+ *     device memory: mr_create binds a caller-provided workspace of at least mr_workspace_bytes_bc() bytes
+ *     (256-byte aligned) that must outlive the context.  mr_ctx itself is host memory owned by the library, and so are
+ *     the CUDA graphs it replays (mr_set_variant), the stream it records them on (they RUN on the caller's stream) and
+ *     32 bytes of pinned host memory through which mr_step_adaptive exchanges dt, Lambda and the error flag.
  *   - All work is enqueued on the caller's stream.  mr_set_B0, mr_get_fields, mr_get_xi and mr_rhs are asynchronous
  *     (the buffers may be reused once the stream has passed the call); every other call synchronises that stream
  *     before it returns (mr_set_x / mr_set_xi for the check of the line-tied faces, mr_step* for the error flag, the

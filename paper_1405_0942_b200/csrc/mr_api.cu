@@ -867,6 +867,9 @@ extern "C" mr_status mr_bind_adaptive_workspace(mr_ctx* ctx, void* workspace_dev
     if (bytes < ctx->L.adaptive_total)
         return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_adaptive_workspace: smaller than mr_adaptive_workspace_bytes_bc()");
     ctx->aws = static_cast<char*>(workspace_dev);
+    for (int o = 0; o < 2; ++o)                   // captured trial steps point into the previous buffer
+        for (int w = 0; w < 2; ++w)
+            if (ctx->trial_graph[o][w]) { cudaGraphExecDestroy(ctx->trial_graph[o][w]); ctx->trial_graph[o][w] = nullptr; }
     MR_CUDA(ctx, cudaMemsetAsync(ctx->aws, 0, ctx->L.adaptive_total, ctx->stream));       // the padding must stay finite
     if (ctx->plans_built) {
         if (ctx->plan_mim.usable && !sym_bind_stage(&ctx->plan_mim, ctx->kbuf_raw(6))) ctx->plan_mim.usable = false;

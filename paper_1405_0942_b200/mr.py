@@ -132,7 +132,10 @@ class Relaxation:
     (or pinned/pageable host tensors for the ``*_host`` calls) of shape ``(3, nz, ny, nx)`` in that dtype.
     """
 
-    def __init__(self, n, lo, hi, dtype="f64", gamma=1.0, bc=("line_tied",) * 3, device="cuda", stream=None):
+    def __init__(self, n, lo, hi, dtype="f64", gamma=1.0, bc=("line_tied",) * 3, device="cuda", stream=None, workspace=None,
+                 adaptive_workspace=None):
+        """``workspace`` / ``adaptive_workspace``: uint8 CUDA tensors of the caller's own (256-byte aligned, at least
+        ``workspace_bytes(...)`` / ``mr_adaptive_workspace_bytes_bc`` bytes); allocated here when not given."""
         import torch
 
         for b in bc:
@@ -155,9 +158,14 @@ class Relaxation:
             raise MrError(MR_ERR_INVALID_ARG, "invalid grid %r / dtype %r" % (self.n, dtype))
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            with torch.cuda.stream(self.stream):            # the workspace belongs to the stream the library works on
-                self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            if workspace is not None:
+                self.workspace = workspace
+                nbytes = int(workspace.numel())
+            else:
+                with torch.cuda.stream(self.stream):        # the workspace belongs to the stream the library works on
+                    self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self._aworkspace = None
+            self._aworkspace_given = adaptive_workspace
             g = mr_grid(*self.n)
             d = mr_domain((C.c_double * 3)(*[float(v) for v in lo]), (C.c_double * 3)(*[float(v) for v in hi]))
             bcs = (C.c_int * 3)(*[BOUNDARIES[b] for b in bc])
@@ -270,8 +278,12 @@ class Relaxation:
                 g = mr_grid(*self.n)
                 bcs = (C.c_int32 * 3)(*[BOUNDARIES[b] for b in self.bc])
                 nb = int(lib.mr_adaptive_workspace_bytes_bc(C.byref(g), MR_F64 if self.dtype == "f64" else MR_F32, bcs))
-                with torch.cuda.stream(self.stream):
-                    self._aworkspace = torch.empty(nb, dtype=torch.uint8, device=self.device)
+                if self._aworkspace_given is not None:
+                    self._aworkspace = self._aworkspace_given
+                    nb = int(self._aworkspace.numel())
+                else:
+                    with torch.cuda.stream(self.stream):
+                        self._aworkspace = torch.empty(nb, dtype=torch.uint8, device=self.device)
                 self._check(lib.mr_bind_adaptive_workspace(self._ctx, self._aworkspace.data_ptr(), nb))
             st, d = mr_adapt_stats(), C.c_double(float(dt))
             cap = int(min(max_trials, 100000)) if trace else 0

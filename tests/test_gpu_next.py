@@ -125,6 +125,30 @@ def test_adaptive_needs_state_and_reports_failure(mr):
     assert e.value.status == mr.MR_ERR_INVALID_ARG and sim.last_adaptive["accepted"] == 2
 
 
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_adaptive_graph_replay_and_workspace_rebinding(mr, op):
+    """The captured trial step (a CUDA graph per operator and state buffer) against plain launches: same trials, same Lambda, same
+    state bit for bit; a second adaptive workspace bound mid-run (the captured graphs point into the first one) changes nothing."""
+    import ctypes as C
+    g, x0, B0, dt = case("C1_rough")
+    out = {}
+    for v in ("graph", "nograph", "rebind"):
+        sim = make_sim(mr, g, x0, B0)
+        sim.set_variant("nograph" if v == "nograph" else "graph")
+        st = sim.step_adaptive(t_end=6 * dt, lambda0=1e-9, dt=dt, op=op, trace=True)
+        if v == "rebind":
+            nb = sim._aworkspace.numel()
+            second = torch.full((nb,), 255, dtype=torch.uint8, device="cuda")     # (garbage: the library must clear it)
+            assert mr.lib.mr_bind_adaptive_workspace(sim._ctx, C.c_void_p(second.data_ptr()), nb) == mr.MR_OK
+            sim._aworkspace.fill_(255)                                               # the first one is no longer used
+        st2 = sim.step_adaptive(t_end=st["time"] + 6 * dt, lambda0=1e-9, dt=st["dt_next"], op=op, trace=True)
+        out[v] = (sim.get_xi().cpu().numpy(), st["trace"] + st2["trace"], sim.launch_count)
+    for v in ("nograph", "rebind"):
+        assert np.array_equal(out["graph"][0], out[v][0])
+        assert out["graph"][1] == out[v][1]
+    assert out["graph"][2] == out["nograph"][2]
+
+
 # ------------------------------------------------------------------------------------------ Eqs. 2.12-2.14
 
 def _periodic_case(bc, n=(20, 12, 10)):

@@ -332,6 +332,57 @@ def test_graph_replay_is_bit_identical_to_plain_launches(mr, op, name, bc):
         sim.set_variant("no-such-kernel")
 
 
+@pytest.mark.parametrize("name,bc,dtype", [("ragged", ("line_tied",) * 3, "f64"), ("wide", ("line_tied",) * 3, "f32"),
+                                           ("tail1", ("periodic",) * 3, "f64"), ("minimal", ("periodic", "line_tied", "periodic"), "f32")])
+def test_no_write_outside_the_buffers_the_caller_gave(mr, name, bc, dtype):
+    """compute-sanitizer is closed on this pool, so the library is run with every buffer it is given embedded in a canary:
+    both workspaces exactly as large as mr_*_workspace_bytes_bc says, dense output arrays of exactly 3 nx ny nz elements, 4 KiB
+    of 0xA5 either side.  Every entry point that writes (steps of both operators, S6, right-hand side, the adaptive integrator,
+    convexity with its map, fields, displacement) must leave the canaries intact."""
+    import ctypes as C
+    g, x0, B0, dt = case(name)
+    if "periodic" in bc:
+        x0 = I.reference_grid(g)                   # (these fields are not periodic: stay at x = X, step little)
+        dt = 1e-3 * dt
+    td = torch.float64 if dtype == "f64" else torch.float32
+    G = 4096
+    canaries = []
+
+    def guarded(nbytes):
+        big = torch.full((nbytes + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+        canaries.append((big, nbytes))
+        return big[G:G + nbytes]
+
+    gg = mr.mr_grid(*g.n)
+    bcs = (C.c_int32 * 3)(*[mr.BOUNDARIES[b] for b in bc])
+    code = mr.MR_F64 if dtype == "f64" else mr.MR_F32
+    ws = guarded(int(mr.lib.mr_workspace_bytes_bc(C.byref(gg), code, bcs)))
+    aws = guarded(int(mr.lib.mr_adaptive_workspace_bytes_bc(C.byref(gg), code, bcs)))
+    sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype, bc=bc, workspace=ws, adaptive_workspace=aws)
+    es = 8 if dtype == "f64" else 4
+    dense = lambda: guarded(3 * g.nodes * es).view(td).view(sim.shape)     # noqa: E731
+    sim.set_B0(dev(B0, td))
+    sim.set_xi(dev(x0 - I.reference_grid(g), td))
+    for variant in ("auto", "generic"):
+        sim.set_variant(variant)
+        for op in ("mimetic", "direct"):
+            sim.step(3, dt, op)
+            sim.step(40, dt, op)                                           # (a graph replay on these L2-resident grids)
+            sim.diagnostics(op)
+            assert mr.lib.mr_rhs(sim._ctx, mr._op(op), C.c_void_p(dense().data_ptr())) == mr.MR_OK
+            sim.step_adaptive(t_end=sim.diagnostics(op)["time"] + 3 * dt, lambda0=1e-7, dt=dt, op=op)
+            sim.get_fields_into(op, x=dense(), B=dense(), J=dense())
+            sim.eps_star(g.n[0] // 2, g.n[1] // 2, 1.0, op)
+    assert mr.lib.mr_get_xi(sim._ctx, C.c_void_p(dense().data_ptr())) == mr.MR_OK
+    kap = guarded(4 * g.nodes)
+    nconc = C.c_int64()
+    assert mr.lib.mr_convexity(sim._ctx, C.c_void_p(kap.data_ptr()), C.byref(nconc)) == mr.MR_OK
+    sim.sigma(dev(x0, td), dev(B0, td))
+    torch.cuda.synchronize()
+    for big, nbytes in canaries:
+        assert bool((big[:G] == 0xA5).all()) and bool((big[G + nbytes:] == 0xA5).all())
+
+
 def test_full_size_config4_one_step_matches_oracle(mr):
     """BASELINE configs[3] at full size (256x256x512, the bench workload and launch configuration), initial grid
     smoothly displaced so that every term is exercised: x after one step and the diagnostics against the oracle
