@@ -225,7 +225,10 @@ def test_fp32_variant_within_1e5_of_fp64(mr, variant):
 
 def test_fp32_variant_full_size_config5(mr):
     """BASELINE configs[4] at full size (512^3, the launch configuration bench.py --workload C5 times): the fp32 context
-    against an fp64 context on the same inputs, 100 steps each; x, B and J within 1e-5 norm-wise."""
+    against an fp64 context on the same inputs.  After 100 steps x, B and J are within 1e-5 norm-wise (Q19).  After the
+    config's 1000 steps the state (x, the displacement itself, B) still is; J, a second difference of a state that has by then
+    been rounded to fp32 a thousand times, is not: its deviation grows like the square root of the step count (measured
+    6.3e-6, 1.37e-5, 2.04e-5 after 100, 500, 1000 steps) and is held to 3e-5 (Q15)."""
     cfg = I.CONFIGS["C5"]
     g = cfg.grid
     x0, B0, dt = I.make(cfg)
@@ -235,22 +238,33 @@ def test_fp32_variant_full_size_config5(mr):
     for dtype, td in (("f64", torch.float64), ("f32", torch.float32)):
         s = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype)
         s.set_B0(B0t.to("cuda", dtype=td))
-        s.step(100, dt)                                     # starts at x = X: no mr_set_x
-        sims[dtype] = s
+        sims[dtype] = s                                     # starts at x = X: no mr_set_x
+
+    def deviations():
+        xi64, xi32 = sims["f64"].get_xi(), sims["f32"].get_xi()
+        errs = {"x": float((xi32.double() - xi64).abs().max()) / 4.0, "xi": rel_dev(xi32, xi64)}
+        del xi64, xi32
+        for name in ("B", "J"):
+            a = sims["f32"].get_fields("mimetic", **{name: True})[name]
+            b = sims["f64"].get_fields("mimetic", **{name: True})[name]
+            errs[name] = rel_dev(a, b)
+            del a, b
+        return errs
+
+    for s in sims.values():
+        s.step(100, dt)
     assert sims["f32"].step_variant == "sym_tmem_f32" and sims["f64"].step_variant == "sym_tmem_f64"
-    xi64, xi32 = sims["f64"].get_xi(), sims["f32"].get_xi()
-    err_x = float((xi32.double() - xi64).abs().max()) / 4.0
-    err_xi = rel_dev(xi32, xi64)
-    del xi64, xi32
-    errs = {"x": err_x, "xi": err_xi}
-    for name in ("B", "J"):
-        a = sims["f32"].get_fields("mimetic", **{name: True})[name]
-        b = sims["f64"].get_fields("mimetic", **{name: True})[name]
-        errs[name] = rel_dev(a, b)
-        del a, b
-    print("fp32 vs fp64 at 512^3 after 100 steps:", errs)
-    assert errs["x"] < TOL_F32 and errs["B"] < TOL_F32 and errs["J"] < TOL_F32, errs
-    assert errs["xi"] < 1e-3, errs
+    e100 = deviations()
+    print("fp32 vs fp64 at 512^3 after 100 steps:", e100)
+    assert e100["x"] < TOL_F32 and e100["B"] < TOL_F32 and e100["J"] < TOL_F32 and e100["xi"] < TOL_F32, e100
+    for s in sims.values():
+        s.step(cfg.steps - 100, dt)
+    e1000 = deviations()
+    print("... after %d steps:" % cfg.steps, e1000)
+    assert e1000["x"] < TOL_F32 and e1000["B"] < TOL_F32 and e1000["xi"] < TOL_F32, e1000
+    assert e1000["J"] < 3e-5, e1000
+    d64, d32 = sims["f64"].diagnostics(), sims["f32"].diagnostics()
+    assert d32["energy"] == pytest.approx(d64["energy"], rel=1e-6) and d32["xi"] == pytest.approx(d64["xi"], rel=1e-4)
 
 
 def test_host_buffer_entry_points_round_trip(mr):
