@@ -346,6 +346,7 @@ def run_ours(args):
                     "hbm_frac": BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9 / peak}
         achieved = BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9
         return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "frac_of_datasheet_8000": achieved / 8000.0,
                 "traffic": recorded_traffic(cfg.name, variant), "peak_source": peak_src, "kernel": variant,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE[dtype] * nodes, "launch_ms": launch_ms}
 
