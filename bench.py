@@ -450,6 +450,20 @@ def paper_table_4_1(phi_over_pi=0.25):
     return rows
 
 
+def paper_table_4_2():
+    """TABLE 4.2 of the paper as printed (tests/golden/paper_table_4_2.txt): {(method, n): (xi, eps*)}, Pontin09, phi = pi/2"""
+    rows = {}
+    try:
+        with open(os.path.join(ROOT, "tests", "golden", "paper_table_4_2.txt")) as f:
+            for line in f:
+                line = line.split("#", 1)[0].split()
+                if line:
+                    rows[(line[0], int(line[1]))] = (float(line[2]), float(line[3]), None, None)
+    except OSError:
+        pass
+    return rows
+
+
 def run_isohelix(args):
     """--isohelix N[,N..]: the paper's own experiment (section 3.1, TABLE 4.1): the IsoHelix field (phi = pi/4) on N^3 nodes relaxed
     with the adaptive Cash-Karp integrator (section 2.4) to t = --t-end, where eps*, sigma_B, sigma_x have stabilised; prints them
@@ -459,13 +473,15 @@ def run_isohelix(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the relaxation step has no CPU path")
     from paper_1405_0942_b200 import inputs as I, mr
-    paper = paper_table_4_1(args.phi)
+    pontin = args.field == "pontin09"
+    paper = (paper_table_4_2() if args.phi == 0.5 else {}) if pontin else paper_table_4_1(args.phi)
     rows, total_rhs, total_s, launches = [], 0, 0.0, 0
     phi = np.pi * args.phi
     td = torch.float64 if args.dtype == "f64" else torch.float32
     for n in [int(v) for v in args.isohelix.split(",")]:
         g = I.Grid((n, n, n), (-4.0, -4.0, -10.0), (4.0, 4.0, 10.0))
-        B0 = I.isohelix_B0(g, phi)
+        # Pontin09 (Eq. 3.4): two twist regions of opposite sense at Z = -+4 (reading Q25)
+        B0 = I.pontin09_B0(g, (phi, -phi), (-4.0, 4.0)) if pontin else I.isohelix_B0(g, phi)
         Bref = np.zeros(g.shape)
         Bref[2] = 1.0
         for op in args.operator.split(","):
@@ -493,7 +509,7 @@ def run_isohelix(args):
             pk = paper.get(("mimetic" if op == "mimetic" else "classic", n))
             rows.append({"n": n, "operator": op, "t_end": st["time"], "accepted": st["accepted"], "rejected": st["rejected"],
                          "seconds": el, "us_per_trial": el / max(st["accepted"] + st["rejected"], 1) * 1e6,
-                         "xi": d["xi"], "eps_star": eps, "sigma_B": sb, "sigma_x": sx, "energy": d["energy"],
+                         "xi": d["xi"], "eps_star": eps, "sigma_B": sb, "sigma_x": None if pontin else sx, "energy": d["energy"],
                          "concave_nodes": sim.convexity()[0], "kernel": sim.step_variant,
                          "paper": None if pk is None else {"xi": pk[0], "eps_star": pk[1], "sigma_B": pk[2], "sigma_x": pk[3]}})
             total_rhs += st["rhs_evals"] * g.nodes
@@ -502,9 +518,10 @@ def run_isohelix(args):
             sim.close()
     line = {"metric": "node right-hand-side evaluations/s (IsoHelix relaxation, adaptive RK5(4), fp64)", "value": total_rhs / max(total_s, 1e-9),
             "unit": "node-rhs/s", "n_gpus": 1, "higher_is_better": True, "dtype": args.dtype, "data": "synthetic", "vs_baseline": None,
-            "config": {"workload": "IsoHelix phi=%g pi (PAPER.md:170-186) on n^3 nodes, n in [%s], lambda0=%g, t_end=%g; "
-                                   "paper rows: TABLE 4.1 (the 'classic' rows are the paper's direct method, whose formulas it does "
-                                   "not print: context only)" % (args.phi, args.isohelix, args.lambda0, args.t_end)},
+            "config": {"workload": "%s phi=%g pi (PAPER.md:170-198) on n^3 nodes, n in [%s], lambda0=%g, t_end=%g; "
+                                   "paper rows: TABLE %s (the 'classic' rows are the paper's direct method, whose formulas it does "
+                                   "not print: context only)" % ("Pontin09 (twists at Z=-+4)" if pontin else "IsoHelix", args.phi,
+                                                                 args.isohelix, args.lambda0, args.t_end, "4.2" if pontin else "4.1")},
             "gpu_launches": launches, "table_4_1": rows}
     print(json.dumps(line))
     return 0
@@ -521,6 +538,7 @@ def main(argv=None):
     ap.add_argument("--operator", default="mimetic", help="mimetic | direct (--isohelix: a comma-separated list of them)")
     ap.add_argument("--isohelix", default="", help="N[,N..]: relax the paper's IsoHelix field on N^3 nodes and report TABLE 4.1's measures")
     ap.add_argument("--t-end", type=float, default=512.0, help="--isohelix: end time of the relaxation")
+    ap.add_argument("--field", default="isohelix", choices=["isohelix", "pontin09"], help="--isohelix: Eq. 3.1 or Eq. 3.4 (TABLE 4.2, use --phi 0.5)")
     ap.add_argument("--phi", type=float, default=0.25, help="--isohelix: twist angle in units of pi (the paper: 0.25, 0.5, 1)")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"], help="--isohelix: precision of the context")
     ap.add_argument("--integrator", default="euler", choices=["euler", "adaptive"])

@@ -191,6 +191,20 @@ def isohelix_x_relax(g: Grid, phi: float, a_r: float = float(np.sqrt(2.0)), a_z:
     return out
 
 
+def pontin09_B0(g: Grid, phi: Sequence[float], L: Sequence[float], B0: float = 1.0, a_r: float = float(np.sqrt(2.0)),
+                a_z: float = 2.0) -> np.ndarray:
+    """Eq. 3.4 (PAPER.md:190): ``B = B0 z^ + sum_i (2 B0 phi_i / (pi a_r)) exp(-(X^2+Y^2)/a_r^2 - (Z-L_i)^2/a_z^2) (-Y, X, 0)``;
+    ``L_i`` = positions of the twist regions along z (the paper does not print them: DESIGN.md reading Q25)."""
+    X = reference_grid(g)
+    out = np.zeros_like(X)
+    out[2] = B0
+    for ph, Li in zip(phi, L):
+        c = 2.0 * B0 * ph / (np.pi * a_r) * np.exp(-(X[0] ** 2 + X[1] ** 2) / a_r ** 2 - (X[2] - Li) ** 2 / a_z ** 2)
+        out[0] += -c * X[1]
+        out[1] += c * X[0]
+    return out
+
+
 # ----------------------------------------------------------------------------------------------------------
 # The five BASELINE.json configurations
 # ----------------------------------------------------------------------------------------------------------
