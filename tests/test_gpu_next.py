@@ -379,6 +379,38 @@ def test_pontin09_relaxation_reproduces_table_4_2(mr, golden_dir, n):
     assert d["xi"] < 1e-4 and abs(d["energy"] - 640.0) < 0.02
 
 
+def test_pontin09_phi_pi_breaks_down_after_the_grid_turns_concave(mr):
+    """Section 4.4 / Figs. 4.3-4.4: for the Pontin09 field with phi_1,2 = +-pi the mimetic scheme "breaks down
+    shortly after the grid becomes locally concave", with "a drop of the time step by several orders of magnitude, at which point
+    the simulation is stopped", while the classical scheme stays stable without improving eps*.  Here on 33^3: kappa = -1 nodes
+    (Eq. 3.11, mr_convexity) appear between t = 20 and t = 60, the adaptive integrator gives up at t = 122 (MR_ERR_NUMERIC, step
+    length collapsed); the direct operator runs on with eps* = 0.62 (65^3: concave from t = 80, break-down at t = 273:
+    "increased grid resolution can delay this blow up")."""
+    n = 33
+    g = I.Grid((n, n, n), (-4.0, -4.0, -10.0), (4.0, 4.0, 10.0))
+    B0 = I.pontin09_B0(g, (np.pi, -np.pi), (-4.0, 4.0))
+    sim = make_sim(mr, g, I.reference_grid(g), B0)
+    t, dt, first_concave, failed_at = 0.0, 1e-3, None, None
+    while t < 300.0:
+        try:
+            st = sim.step_adaptive(t_end=t + 20.0, lambda0=1e-8, dt=dt, max_trials=300000)
+        except mr.NumericError:
+            failed_at = sim.last_adaptive["time"]
+            assert sim.last_adaptive["dt_next"] < 1e-6 * dt           # the step length collapsed by orders of magnitude
+            break
+        t, dt = st["time"], st["dt_next"]
+        if first_concave is None and sim.convexity()[0] > 0:
+            first_concave = t
+    assert first_concave is not None and failed_at is not None and first_concave < failed_at, (first_concave, failed_at)
+    assert 60.0 < failed_at < 250.0
+    with pytest.raises(mr.MrError):                                   # the context stays failed until a new state is set
+        sim.step(1, 1e-3)
+    direct = make_sim(mr, g, I.reference_grid(g), B0)
+    st = direct.step_adaptive(t_end=200.0, lambda0=1e-8, dt=1e-3, op="direct", max_trials=300000)
+    _, eps = direct.eps_star(n // 2, n // 2, np.sqrt(2.0), "direct")
+    assert st["time"] == 200.0 and eps > 0.3 and direct.diagnostics("direct")["xi"] < 1e-3
+
+
 def test_isohelix_relaxation_on_the_gpu_follows_the_oracle(mr):
     """The same run at n = 17 on both sides to t = 64 (the oracle's Lambda is |x5 - x4|, the library's the weighted stage sum:
     the two agree to ~1e-7, so near Lambda0 a trial may be judged differently and the step sequences part; the states they
