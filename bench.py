@@ -58,11 +58,12 @@ def measured_peak_gbs():
 
 
 def csrc_fingerprint():
-    """sha1 over the CUDA sources: a traffic row is only valid for the sources it was captured with."""
+    """sha1 over the device code (csrc/*.cuh: the kernels, their layouts and the launch geometry): a traffic row is only valid for
+    the kernels it was captured with.  (mr_api.cu, the host side of the ABI, does not enter.)"""
     import glob
     import hashlib
     h = hashlib.sha1()
-    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1405_0942_b200", "csrc", "*"))):
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1405_0942_b200", "csrc", "*.cuh"))):
         with open(f, "rb") as fh:
             h.update(os.path.basename(f).encode() + b"\0" + fh.read())
     return h.hexdigest()[:16]
