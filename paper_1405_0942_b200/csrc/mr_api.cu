@@ -422,7 +422,8 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     const int threads = c->grid.nx >= 256 ? 256 : (c->grid.nx >= 128 ? 128 : (c->grid.nx >= 64 ? 64 : 32));
     const bool stream_ok = streaming(c, op);
     const StreamPlan& pl = op == MR_OP_MIMETIC ? c->plan_mim : c->plan_dir;
-    const bool fused = stream_ok && pl.tiles_x * pl.tiles_y * pl.nchunks <= kMaxPartialBlocks;
+    const Tiling& tl = op == MR_OP_MIMETIC ? pl.all : pl.step;
+    const bool fused = stream_ok && tl.tiles_x * tl.tiles_y * tl.nchunks <= kMaxPartialBlocks;
     int total = blocks;
     if (fused && op == MR_OP_MIMETIC) {
         // the streaming pass of the step kernel with the update replaced by the reduction (mr_sym.cuh, MODE_DIAG)

@@ -133,7 +133,7 @@ k_step_direct(const __grid_constant__ CUtensorMap map_in, const __grid_constant_
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x % a.ntiles, chunk = blockIdx.x / a.ntiles;
-    const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY;
+    const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY + a.jorg;
     const int nz = a.nz;
     const int k0 = chunk * a.chunk_len, k1 = min(k0 + a.chunk_len, nz);
     // a periodic axis (Eqs. 2.12-2.14) has no face: its ghost layers sit in the padded arrays, every node is an inner point
@@ -260,8 +260,6 @@ inline bool build_direct_plan(StreamPlan* p, const StreamGeom& g, bool f64, void
         *why = "cuTensorMapEncodeTiled failed";
         return false;
     }
-    p->tiles_x = (g.nx + Ld::TX - 1) / Ld::TX;
-    p->tiles_y = (g.ny + kXTY - 1) / kXTY;
     p->smem_bytes = f64 ? Ld::BYTES : Lf::BYTES;
     cudaError_t e = cudaSuccess;
     const int sb = (int)p->smem_bytes;
@@ -278,7 +276,7 @@ inline bool build_direct_plan(StreamPlan* p, const StreamGeom& g, bool f64, void
         *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
         return false;
     }
-    choose_chunks(p->tiles_x * p->tiles_y, g.nz, sm_count, &p->nchunks, &p->chunk_len);
+    choose_tilings(p, Ld::TX, kXTY, false, sm_count);
     p->usable = true;
     return true;
 }
@@ -296,9 +294,9 @@ template <typename T>
 inline cudaError_t launch_direct_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream, bool rhs = false, void* out = nullptr)
 {
     using L = DirectLayout<T, kXTY, kXR>;
-    const StreamArgs<T> a = stream_args<T>(p, dtg, flag);
+    const StreamArgs<T> a = stream_args<T>(p, p.step, dtg, flag);
     T* o = static_cast<T*>(out ? out : p.xi[1 - cur]);
-    const int grid = a.ntiles * p.nchunks;
+    const int grid = a.ntiles * p.step.nchunks;
     if (rhs) k_step_direct<T, kXTY, kXR, 2><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, o, a);
     else k_step_direct<T, kXTY, kXR, 0><<<grid, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, o, a);
     return cudaGetLastError();
@@ -309,8 +307,8 @@ template <typename T>
 inline cudaError_t launch_direct_diag(const StreamPlan& p, int cur, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
 {
     using L = DirectLayout<T, kXTY, kXR>;
-    const StreamArgs<T> a = stream_args<T>(p, (T)0, flag);
-    *nblocks = a.ntiles * p.nchunks;
+    const StreamArgs<T> a = stream_args<T>(p, p.step, (T)0, flag);       // (the nodes on the faces are k_diag_faces' anyway)
+    *nblocks = a.ntiles * p.step.nchunks;
     k_step_direct<T, kXTY, kXR, 1><<<*nblocks, L::NTHREADS, p.smem_bytes, stream>>>(p.map_xi[cur], p.map_b, reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();
 }

@@ -35,9 +35,19 @@ struct StreamArgs {
     T twoh[3];
     T dtg;
     int tiles_x, ntiles, chunk_len;
+    int jorg;             // row of the first tile: 1 when the line-tied face row j = 0 is left to the halo ring (see Tiling)
     int ox, oy, oz;       // box coordinate of the node (0, 0, 0) in the tensor maps (= the ghost widths)
     int per;              // bit a: axis a is periodic (no face, no one-sided difference, every node an inner point)
     int* flag;
+};
+
+// How the xy plane is cut into tiles.  `all`: every node is a tile node (what S6 needs: it sums over all of them).  `step`:
+// the nodes on LINE-TIED faces never move and both state buffers hold their zero displacement for good, so a step (or a
+// right-hand side) need not own them: the tiles start at row 1, and a face that falls exactly one node past the last tile is
+// served by that tile's halo ring (mimetic) or by nobody (direct).  On the paper's grids of 2^m + 1 nodes that is 4 x 8 tiles
+// instead of 5 x 9 (129^2), 2 x 4 instead of 3 x 5 (65^2), 1 x 2 instead of 2 x 3 (33^2).
+struct Tiling {
+    int tiles_x = 0, tiles_y = 0, nchunks = 0, chunk_len = 0, jorg = 0;
 };
 
 struct StreamPlan {
@@ -50,7 +60,7 @@ struct StreamPlan {
     CUtensorMap map_b;
     void* xi[3] = { nullptr, nullptr, nullptr };
     const void* b = nullptr;
-    int tiles_x = 0, tiles_y = 0, nchunks = 0, chunk_len = 0;
+    Tiling all, step;
     size_t smem_bytes = 0;
 };
 
@@ -248,17 +258,38 @@ inline void choose_chunks(int ntiles, int nz, int slots, int* nchunks, int* chun
 }
 
 
+// the two tilings of a plan: tx / ty = tile size, ring = the kernel forms B on the halo-1 ring of a tile (mimetic)
+inline void choose_tilings(StreamPlan* p, int tx, int ty, bool ring, int sm_count)
+{
+    const StreamGeom& g = p->g;
+    p->all.tiles_x = (g.nx + tx - 1) / tx;
+    p->all.tiles_y = (g.ny + ty - 1) / ty;
+    p->all.jorg = 0;
+    p->step = p->all;
+    if (!g.per[0]) {
+        if (ring) { if ((g.nx - 1) % tx == 0) p->step.tiles_x = (g.nx - 1) / tx; }
+        else p->step.tiles_x = (g.nx - 1 + tx - 1) / tx;
+    }
+    if (!g.per[1] && (g.ny - 2 + ty - 1) / ty < p->all.tiles_y) {
+        p->step.tiles_y = (g.ny - 2 + ty - 1) / ty;
+        p->step.jorg = 1;
+    }
+    choose_chunks(p->all.tiles_x * p->all.tiles_y, g.nz, sm_count, &p->all.nchunks, &p->all.chunk_len);
+    choose_chunks(p->step.tiles_x * p->step.tiles_y, g.nz, sm_count, &p->step.nchunks, &p->step.chunk_len);
+}
+
 template <typename T>
-inline StreamArgs<T> stream_args(const StreamPlan& p, T dtg, int* flag)
+inline StreamArgs<T> stream_args(const StreamPlan& p, const Tiling& t, T dtg, int* flag)
 {
     StreamArgs<T> a;
     a.nx = p.g.nx; a.ny = p.g.ny; a.nz = p.g.nz;
     a.pitch = p.g.pitch; a.plane = p.g.plane; a.comp = p.g.comp;
     for (int c = 0; c < 3; ++c) a.twoh[c] = (T)p.g.twoh[c];
     a.dtg = dtg;
-    a.tiles_x = p.tiles_x;
-    a.ntiles = p.tiles_x * p.tiles_y;
-    a.chunk_len = p.chunk_len;
+    a.tiles_x = t.tiles_x;
+    a.ntiles = t.tiles_x * t.tiles_y;
+    a.chunk_len = t.chunk_len;
+    a.jorg = t.jorg;
     a.ox = p.g.ghost[0]; a.oy = p.g.ghost[1]; a.oz = p.g.ghost[2];
     a.per = (p.g.per[0] ? 1 : 0) | (p.g.per[1] ? 2 : 0) | (p.g.per[2] ? 4 : 0);
     a.flag = flag;

@@ -105,7 +105,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool tilew = warp < NTW;
     const int tile = blockIdx.x % a.ntiles, chunk = blockIdx.x / a.ntiles;
-    const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY;
+    const int i0 = (tile % a.tiles_x) * TX, j0 = (tile / a.tiles_x) * TY + a.jorg;
     const int nz = a.nz;
     // a periodic axis (Eqs. 2.12-2.14) has no face: its ghost layers (two planes / rows, 16 bytes of columns either side) sit
     // in the padded arrays, B is formed on the first ghost layer like on any halo node, and every node is an inner point
@@ -515,9 +515,6 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
         *why = "cuTensorMapEncodeTiled failed";
         return false;
     }
-    const int tx = f64 ? Ld::TX : Lf::TX;
-    p->tiles_x = (g.nx + tx - 1) / tx;
-    p->tiles_y = (g.ny + Ld::TY - 1) / Ld::TY;
     p->smem_bytes = f64 ? Ld::BYTES : Lf::BYTES;
     cudaError_t e = cudaSuccess;
     const int sb = (int)p->smem_bytes;
@@ -529,7 +526,7 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
         *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
         return false;
     }
-    choose_chunks(p->tiles_x * p->tiles_y, g.nz, sm_count, &p->nchunks, &p->chunk_len);
+    choose_tilings(p, f64 ? Ld::TX : Lf::TX, Ld::TY, true, sm_count);
     p->usable = true;
     return true;
 }
@@ -548,9 +545,9 @@ inline bool sym_bind_stage(StreamPlan* p, void* xs)
 template <typename T>
 inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* flag, cudaStream_t stream, bool rhs = false, void* out = nullptr)
 {
-    const StreamArgs<T> a = stream_args<T>(p, dtg, flag);
+    const StreamArgs<T> a = stream_args<T>(p, p.step, dtg, flag);
     T* o = static_cast<T*>(out ? out : p.xi[1 - cur]);
-    sym_kernel<T>(rhs ? MODE_RHS : MODE_STEP, a.per != 0)<<<a.ntiles * p.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+    sym_kernel<T>(rhs ? MODE_RHS : MODE_STEP, a.per != 0)<<<a.ntiles * p.step.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
         p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), o, a);
     return cudaGetLastError();
 }
@@ -559,8 +556,8 @@ inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* fla
 template <typename T>
 inline cudaError_t launch_sym_diag(const StreamPlan& p, int cur, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
 {
-    const StreamArgs<T> a = stream_args<T>(p, (T)0, flag);
-    *nblocks = a.ntiles * p.nchunks;
+    const StreamArgs<T> a = stream_args<T>(p, p.all, (T)0, flag);
+    *nblocks = a.ntiles * p.all.nchunks;
     sym_kernel<T>(MODE_DIAG, a.per != 0)<<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
         p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), reinterpret_cast<T*>(partials), a);
     return cudaGetLastError();

@@ -70,6 +70,15 @@ def case(name):
         g = I.Grid((17, 17, 21), (-4.0, -4.0, -10.0), (4.0, 4.0, 10.0))
         B0 = I.isohelix_B0(g, np.pi / 4)
         return g, I.displaced_grid(g, 0.25, seed=13), B0, 0.5 * I.stable_dt(B0, g)
+    if name == "pow2p1":        # 2^m + 1 nodes in x and y (the paper's grids): the step tiling leaves the line-tied faces i = nx-1
+                                # and j = 0 to the halo ring of the tiles (Tiling, mr_stream_common.cuh)
+        g = I.Grid((33, 33, 11), (-4.0, -4.0, -5.0), (4.0, 4.0, 5.0))
+        B0 = I.isohelix_B0(g, np.pi / 2)
+        return g, I.displaced_grid(g, 0.25, seed=21), B0, 0.5 * I.stable_dt(B0, g)
+    if name == "pow2p1_wide":   # ... with nx - 1 = 64 (the fp32 kernel's tile width) and several tiles in x
+        g = I.Grid((129, 17, 9), (-8.0, -2.0, -2.0), (8.0, 2.0, 2.0))
+        B0 = I.twist_field(g, (I.Twist(1.0, 2.0, 0.0, 0.0), I.Twist(-1.0, -3.0, 0.5, 0.5)))
+        return g, I.displaced_grid(g, 0.3, seed=23), B0, 0.5 * I.stable_dt(B0, g)
     if name == "C2_small":      # config 2 field at a quarter of the resolution
         cfg = I.scaled(I.CONFIGS["C2"], (32, 32, 96))
         x0, B0, dt = I.make(cfg)
@@ -81,7 +90,7 @@ def case(name):
     raise KeyError(name)
 
 
-CASES = ["C1", "C1_rough", "ragged", "minimal", "wide", "tail1", "C2_small", "C3_small"]
+CASES = ["C1", "C1_rough", "ragged", "minimal", "wide", "tail1", "pow2p1", "pow2p1_wide", "C2_small", "C3_small"]
 
 
 def opcode(op):

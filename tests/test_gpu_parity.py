@@ -223,6 +223,25 @@ def test_fp32_variant_within_1e5_of_fp64(mr, variant):
     assert d32["energy"] == pytest.approx(d64["energy"], rel=TOL_F32)
 
 
+@pytest.mark.parametrize("name", ["pow2p1", "pow2p1_wide", "tail1", "ragged"])
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_fp32_steps_on_ragged_and_face_ring_tilings(mr, name, op):
+    """The fp32 kernels (two nodes per thread, 64-wide tiles) on grids whose faces fall on tile edges, ring columns and ragged
+    tails: 20 steps against the oracle through the displacement (Q15), and the faces stay exactly where they are."""
+    g, x0, B0, dt = case(name)
+    sim = make_sim(mr, g, x0, B0, dtype="f32")
+    sim.step(20, dt, op)
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 20, op=opcode(op))
+    X = I.reference_grid(g)
+    xi = sim.get_xi().double().cpu().numpy()
+    assert np.abs(xi - (ref - X)).max() < 3 * TOL_F32 * np.abs(ref - X).max()
+    m = np.ones(xi.shape, bool)
+    m[:, 1:-1, 1:-1, 1:-1] = False
+    assert not xi[m].any()
+    f = sim.get_fields(op, B=True)["B"].double().cpu().numpy()
+    assert nrel(f, mro.fields(g.n, g.lo, g.hi, ref, B0, op=opcode(op))[0]) < 3 * TOL_F32
+
+
 def test_fp32_variant_full_size_config5(mr):
     """BASELINE configs[4] at full size (512^3, the launch configuration bench.py --workload C5 times): the fp32 context
     against an fp64 context on the same inputs.  After 100 steps x, B and J are within 1e-5 norm-wise (Q19).  After the
