@@ -106,7 +106,7 @@ struct mr_ctx {
     cudaGraphExec_t trial_graph[2][2] = { { nullptr, nullptr }, { nullptr, nullptr } };
     int tg_variant[2][2] = { { -1, -1 }, { -1, -1 } };
     int64_t tg_launches[2][2] = { { 0, 0 }, { 0, 0 } };
-    double* pinned = nullptr;              // [0] dt of the trial, [1] Lambda, [2] the flag word (as an int)
+    double* pinned = nullptr;              // [0] dt of the trial, [1] the flag word (as an int), [2] Lambda
     std::string err;
 
     ~mr_ctx()
@@ -130,6 +130,7 @@ struct mr_ctx {
     DiagPartial* partials() const { return reinterpret_cast<DiagPartial*>(ws + L.off_partials); }
     DiagPartial* diag_out() const { return reinterpret_cast<DiagPartial*>(ws + L.off_diag); }
     int* flag() const { return reinterpret_cast<int*>(ws + L.off_flag); }
+    double* lambda_dev() const { return reinterpret_cast<double*>(ws + L.off_flag + 8); }   // next to the flag: one memset, one copy
     double* dt_dev() const { return reinterpret_cast<double*>(ws + L.off_diag + 128); }   // the trial step length (kernels read it)
     void* kbuf_raw(int s) const { return aws + (size_t)s * L.field_bytes; }  // s = 0..5: k_1..k_6, 6: the stage state
     void* kbuf(int s) const { return aws + (size_t)s * L.field_bytes + node0(); }
@@ -464,7 +465,7 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
 
 // ---- section 2.4: one Cash-Karp trial step from the state buffer `cur`; the fifth-order solution goes to the other
 // state buffer.  Everything is enqueued on c->stream and nothing depends on the step length, which the kernels read from
-// dt_dev(): pinned[0] -> dt_dev() goes in first, Lambda = max |x5 - x4| -> pinned[1] and the flag -> pinned[2] come out last.
+// dt_dev(): pinned[0] -> dt_dev() goes in first, the flag -> pinned[1] and Lambda = max |x5 - x4| -> pinned[2] come out last.
 template <typename T>
 mr_status enqueue_trial(mr_ctx* c, mr_operator op)
 {
@@ -473,7 +474,7 @@ mr_status enqueue_trial(mr_ctx* c, mr_operator op)
     const int blocks = c->sm_count * 8 < kMaxPartialBlocks ? c->sm_count * 8 : kMaxPartialBlocks;
     const T* x = static_cast<const T*>(c->xi_raw(c->cur));      // the elementwise kernels run over the whole padded fields
     T* xs = static_cast<T*>(c->kbuf_raw(6));
-    MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
+    MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, 16, c->stream));                  // the flag and Lambda (an atomic maximum from 0)
     MR_CUDA(c, cudaMemcpyAsync(c->dt_dev(), c->pinned, sizeof(double), cudaMemcpyHostToDevice, c->stream));
     for (int s = 0; s < 6; ++s) {
         if (s > 0) {
@@ -490,14 +491,11 @@ mr_status enqueue_trial(mr_ctx* c, mr_operator op)
     StageArgs b5, db;
     b5.n = db.n = 6;
     for (int r = 0; r < 6; ++r) { b5.k[r] = db.k[r] = c->kbuf_raw(r); b5.c[r] = ck.b5[r]; db.c[r] = ck.db[r]; }
-    double* partial = reinterpret_cast<double*>(c->partials());
-    k_rk_final<T><<<blocks, 256, 0, c->stream>>>(x, static_cast<T*>(c->xi_raw(1 - c->cur)), b5, db, n2, partial, c->dt_dev());
-    k_max_final<<<1, 256, 0, c->stream>>>(partial, blocks, reinterpret_cast<double*>(c->diag_out()));
-    c->launches += 2;
+    k_rk_final<T><<<blocks, 256, 0, c->stream>>>(x, static_cast<T*>(c->xi_raw(1 - c->cur)), b5, db, n2, c->lambda_dev(), c->dt_dev());
+    c->launches++;
     wrap_ghosts<T>(c, c->xi(1 - c->cur));
     MR_CUDA(c, cudaGetLastError());
-    MR_CUDA(c, cudaMemcpyAsync(c->pinned + 1, c->diag_out(), sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    MR_CUDA(c, cudaMemcpyAsync(c->pinned + 2, c->flag(), sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaMemcpyAsync(c->pinned + 1, c->flag(), 16, cudaMemcpyDeviceToHost, c->stream));    // the flag, Lambda
     return MR_OK;
 }
 
@@ -552,8 +550,8 @@ mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* num
         if (st != MR_OK) return st;
     }
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
-    *lambda = c->pinned[1];
-    *numeric = *reinterpret_cast<const int*>(c->pinned + 2);
+    *numeric = *reinterpret_cast<const int*>(c->pinned + 1);
+    *lambda = c->pinned[2];
     return MR_OK;
 }
 

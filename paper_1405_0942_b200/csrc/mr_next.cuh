@@ -61,7 +61,7 @@ k_rk_stage(const T* __restrict__ xi, T* __restrict__ xs, StageArgs a, long long 
     }
 }
 
-// xi5 = xi + sum_s (dt b_s) k_s, and the block's maximum of |x5 - x4| = |sum_s dt (b_s - b*_s) k_s| ("the maximum error in
+// xi5 = xi + sum_s (dt b_s) k_s, and (into *partial, zeroed by the caller) the grid's maximum of |x5 - x4| = |sum_s dt (b_s - b*_s) k_s| ("the maximum error in
 // x").  A maximum does not depend on the order: the result is deterministic.
 template <typename T>
 __global__ void __launch_bounds__(256)
@@ -102,28 +102,9 @@ k_rk_final(const T* __restrict__ xi, T* __restrict__ x5, StageArgs b5, StageArgs
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int w = 1; w < (int)(blockDim.x >> 5); ++w) lam = (sh[w] > lam || sh[w] != sh[w]) ? sh[w] : lam;
-        partial[blockIdx.x] = lam;
-    }
-}
-
-__global__ void k_max_final(const double* __restrict__ partial, int n, double* __restrict__ out)
-{
-    double lam = 0.0;
-    for (int q = threadIdx.x; q < n; q += blockDim.x) {
-        const double w = partial[q];
-        lam = (w > lam || w != w) ? w : lam;
-    }
-    __shared__ double sh[8];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        const double w = __shfl_down_sync(0xffffffffu, lam, o);
-        lam = (w > lam || w != w) ? w : lam;
-    }
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = lam;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) lam = (sh[w] > lam || sh[w] != sh[w]) ? sh[w] : lam;
-        *out = lam;
+        // lam >= 0 or NaN: as 64-bit patterns the non-negative doubles order like unsigned integers and a (positive) NaN lies
+        // above +inf, so one atomic maximum per block gives the grid's maximum, NaN winning, whatever the order of the blocks
+        atomicMax(reinterpret_cast<unsigned long long*>(partial), (unsigned long long)__double_as_longlong(fabs(lam)));
     }
 }
 
