@@ -134,6 +134,20 @@ mr_status mr_diagnostics(mr_ctx* ctx, mr_operator op, mr_diag* out);
 mr_status mr_get_fields(mr_ctx* ctx, mr_operator op, void* x_dev, void* B_dev, void* J_dev);
 mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_host, void* B_host, void* J_host);
 
+/* ---- streaming through host buffers: one step of the whole path per call, positions in, positions out ------------------
+ * mr_step_host_async = mr_set_x_host(x_in_host) + mr_step(n, dt, op) + mr_get_fields_host(x = x_out_host), but ASYNCHRONOUS:
+ * it returns once the work is enqueued.  The device->host copy of a call runs on a stream of the library's own and overlaps
+ * the host->device copy of the next call (PCIe is full duplex), so a sequence of calls moves 2 x 24 nx ny nz bytes per call at
+ * the rate of ONE direction.  Needs a second dense staging field, bound once (caller-owned device memory, 256-byte aligned,
+ * mr_stream_workspace_bytes = 3 nx ny nz elements).  x_in_host / x_out_host: [3][nz][ny][nx] in the context dtype, pinned host
+ * memory (pageable memory works but serialises the copies); both must stay valid and x_out_host unread until mr_host_sync.
+ * mr_host_sync waits for everything enqueued and reports what mr_set_x / mr_step would have: MR_ERR_INVALID_ARG if some
+ * x_in had a line-tied boundary node off the reference grid, MR_ERR_NUMERIC if some state folded (the context is then failed). */
+size_t mr_stream_workspace_bytes(const mr_grid* grid, mr_dtype dtype);
+mr_status mr_bind_stream_workspace(mr_ctx* ctx, void* workspace_dev, size_t bytes);
+mr_status mr_step_host_async(mr_ctx* ctx, const void* x_in_host, void* x_out_host, int64_t n, double dt, mr_operator op);
+mr_status mr_host_sync(mr_ctx* ctx);
+
 /* The velocity u = gamma J x B (Eq. 1.5, :40) of the current state, dense, context dtype, 0 on line-tied boundary
  * nodes: the right-hand side of dx/dt = u that mr_step and mr_step_adaptive integrate.  Asynchronous. */
 mr_status mr_rhs(mr_ctx* ctx, mr_operator op, void* u_dev);

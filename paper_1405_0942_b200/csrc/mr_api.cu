@@ -107,6 +107,11 @@ struct mr_ctx {
     int tg_variant[2][2] = { { -1, -1 }, { -1, -1 } };
     int64_t tg_launches[2][2] = { { 0, 0 }, { 0, 0 } };
     double* pinned = nullptr;              // [0] dt of the trial, [1] the flag word (as an int), [2] Lambda
+    // mr_step_host_async: a second dense staging field (caller-owned), a stream of the library's own for the device -> host copies
+    char* sws = nullptr;
+    cudaStream_t d2h_stream = nullptr;
+    cudaEvent_t ev_fields = nullptr, ev_d2h = nullptr;
+    bool d2h_pending = false, pipeline_open = false;
     std::string err;
 
     ~mr_ctx()
@@ -116,6 +121,9 @@ struct mr_ctx {
             for (int w = 0; w < 2; ++w)
                 if (trial_graph[o][w]) cudaGraphExecDestroy(trial_graph[o][w]);
         if (cap_stream) cudaStreamDestroy(cap_stream);
+        if (d2h_stream) cudaStreamDestroy(d2h_stream);
+        if (ev_fields) cudaEventDestroy(ev_fields);
+        if (ev_d2h) cudaEventDestroy(ev_d2h);
         if (pinned) cudaFreeHost(pinned);
     }
 
@@ -969,6 +977,103 @@ extern "C" mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_hos
     mr_status st = read_flag(ctx, &f);
     if (st != MR_OK) return st;
     if (f & FLAG_NUMERIC) return fail(ctx, MR_ERR_NUMERIC, "mr_get_fields_host: det(dx/dX) <= 0 or a non-finite value was met");
+    return MR_OK;
+}
+
+extern "C" size_t mr_stream_workspace_bytes(const mr_grid* grid, mr_dtype dtype)
+{
+    Layout L;
+    return make_layout(grid, dtype, nullptr, &L) ? L.stage_bytes : 0;
+}
+
+extern "C" mr_status mr_bind_stream_workspace(mr_ctx* ctx, void* workspace_dev, size_t bytes)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) % kAlign) != 0)
+        return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_stream_workspace: workspace is null or not 256-byte aligned");
+    if (bytes < ctx->L.stage_bytes)
+        return fail(ctx, MR_ERR_WORKSPACE, "mr_bind_stream_workspace: smaller than mr_stream_workspace_bytes()");
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_bind_stream_workspace: calls are in flight (mr_host_sync first)");
+    ctx->sws = static_cast<char*>(workspace_dev);
+    return MR_OK;
+}
+
+namespace {
+template <typename T>
+mr_status do_step_host_async(mr_ctx* c, const void* x_in, void* x_out, int64_t n, double dt, mr_operator op)
+{
+    if (!c->d2h_stream) {
+        MR_CUDA(c, cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
+        MR_CUDA(c, cudaEventCreateWithFlags(&c->ev_fields, cudaEventDisableTiming));
+        MR_CUDA(c, cudaEventCreateWithFlags(&c->ev_d2h, cudaEventDisableTiming));
+    }
+    if (!c->pipeline_open) {             // the flag word collects the faults of every call until mr_host_sync reads it
+        MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
+        c->pipeline_open = true;
+    }
+    dim3 grid, block;
+    node_launch_dims(c, grid, block);
+    // host -> device into the staging field of the context, import into the spare state buffer, adopt it
+    MR_CUDA(c, cudaMemcpyAsync(c->stage(), x_in, c->dense_bytes(), cudaMemcpyHostToDevice, c->stream));
+    const int other = 1 - c->cur;
+    k_import_x<T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(c->stage()), static_cast<T*>(c->xi(other)), grid_params<T>(c),
+                                                 domain_params(c), c->flag());
+    c->launches++;
+    wrap_ghosts<T>(c, c->xi(other));
+    c->cur = other;
+    c->time = 0.0;
+    c->steps = 0;
+    mr_status st = launch_steps<T>(c, n, dt * c->gamma, op);
+    if (st != MR_OK) return st;
+    c->time += dt * (double)n;
+    c->steps += n;
+    // the new positions, dense, into the second staging field once the previous call's copy has left it ...
+    if (c->d2h_pending) MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_d2h, 0));
+    k_fields<T, 0><<<grid, block, 0, c->stream>>>(static_cast<const T*>(c->xi(c->cur)), static_cast<const T*>(c->b()), grid_params<double>(c),
+                                                  domain_params(c), reinterpret_cast<T*>(c->sws), nullptr, nullptr, c->flag());
+    c->launches++;
+    MR_CUDA(c, cudaGetLastError());
+    MR_CUDA(c, cudaEventRecord(c->ev_fields, c->stream));
+    // ... and device -> host on the library's stream, while the caller's stream goes on with the next call
+    MR_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, c->ev_fields, 0));
+    MR_CUDA(c, cudaMemcpyAsync(x_out, c->sws, c->dense_bytes(), cudaMemcpyDeviceToHost, c->d2h_stream));
+    MR_CUDA(c, cudaEventRecord(c->ev_d2h, c->d2h_stream));
+    c->d2h_pending = true;
+    return MR_OK;
+}
+}  // namespace
+
+extern "C" mr_status mr_step_host_async(mr_ctx* ctx, const void* x_in_host, void* x_out_host, int64_t n, double dt, mr_operator op)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!x_in_host || !x_out_host) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_host_async: null pointer");
+    if (n < 0 || !(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_host_async: need n >= 0 and finite dt > 0");
+    if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_host_async: unknown operator");
+    if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_step_host_async: B0 has not been set");
+    if (!ctx->sws) return fail(ctx, MR_ERR_STATE, "mr_step_host_async: no stream workspace bound (mr_bind_stream_workspace)");
+    return ctx->dtype == MR_F64 ? do_step_host_async<double>(ctx, x_in_host, x_out_host, n, dt, op)
+                                : do_step_host_async<float>(ctx, x_in_host, x_out_host, n, dt, op);
+}
+
+extern "C" mr_status mr_host_sync(mr_ctx* ctx)
+{
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (!ctx->pipeline_open) return MR_OK;
+    int f = 0;
+    mr_status st = read_flag(ctx, &f);                          // (synchronises the caller's stream)
+    if (st != MR_OK) return st;
+    if (ctx->d2h_stream) MR_CUDA(ctx, cudaStreamSynchronize(ctx->d2h_stream));
+    ctx->pipeline_open = false;
+    ctx->d2h_pending = false;
+    if (f & FLAG_BOUNDARY) {
+        ctx->failed = true;
+        return fail(ctx, MR_ERR_INVALID_ARG, "mr_host_sync: a line-tied boundary node of some x_in was not on the reference grid X");
+    }
+    if (f & FLAG_NUMERIC) {
+        ctx->failed = true;
+        return fail(ctx, MR_ERR_NUMERIC, "mr_host_sync: det(dx/dX) <= 0 or a non-finite value was met");
+    }
+    ctx->failed = false;
     return MR_OK;
 }
 

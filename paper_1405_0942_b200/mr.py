@@ -97,6 +97,11 @@ lib.mr_launch_count.restype = C.c_int64
 lib.mr_step_variant.argtypes = [_ctx_p]
 lib.mr_step_variant.restype = C.c_char_p
 lib.mr_set_variant.argtypes = [_ctx_p, C.c_char_p]
+lib.mr_stream_workspace_bytes.argtypes = [C.POINTER(mr_grid), C.c_int]
+lib.mr_stream_workspace_bytes.restype = C.c_size_t
+lib.mr_bind_stream_workspace.argtypes = [_ctx_p, C.c_void_p, C.c_size_t]
+lib.mr_step_host_async.argtypes = [_ctx_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int]
+lib.mr_host_sync.argtypes = [_ctx_p]
 lib.mr_set_variant.restype = C.c_int
 
 
@@ -335,6 +340,24 @@ class Relaxation:
     @property
     def step_variant(self):
         return (lib.mr_step_variant(self._ctx) or b"").decode()
+
+    def step_host_async(self, x_in, x_out, n, dt, op="mimetic"):
+        """mr_step_host_async: positions in (host tensor), n steps, positions out (host tensor), enqueued without waiting; the
+        copy out overlaps the next call's copy in.  Keep both tensors alive and x_out unread until host_sync()."""
+        torch = self._torch
+        with torch.cuda.device(self.device):
+            if getattr(self, "_sworkspace", None) is None:
+                g = mr_grid(*self.n)
+                nb = int(lib.mr_stream_workspace_bytes(C.byref(g), MR_F64 if self.dtype == "f64" else MR_F32))
+                with torch.cuda.stream(self.stream):
+                    self._sworkspace = torch.empty(nb, dtype=torch.uint8, device=self.device)
+                self._check(lib.mr_bind_stream_workspace(self._ctx, self._sworkspace.data_ptr(), nb))
+            self._check(lib.mr_step_host_async(self._ctx, self._host(x_in, "x_in"), self._host(x_out, "x_out"), int(n), float(dt), _op(op)))
+
+    def host_sync(self):
+        """mr_host_sync: wait for every step_host_async enqueued; raises what mr_set_x / mr_step would have raised."""
+        with self._torch.cuda.device(self.device):
+            self._check(lib.mr_host_sync(self._ctx))
 
     def close(self):
         if getattr(self, "_ctx", None):

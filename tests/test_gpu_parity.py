@@ -300,6 +300,50 @@ def test_host_buffer_entry_points_round_trip(mr):
     assert nrel(out["J"].numpy(), J) < 1e-10
 
 
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_streaming_host_calls_equal_the_synchronous_ones(mr, op, dtype):
+    """mr_step_host_async / mr_host_sync: six calls in flight (the copy out of one overlapping the copy in of the next, pinned
+    buffers) give bit for bit what mr_set_x_host + mr_step + mr_get_fields_host give one after the other; a state whose
+    line-tied faces are off the reference grid is reported by the sync, and so is a folded grid."""
+    g, x0, B0, dt = case("ragged")
+    td = torch.float64 if dtype == "f64" else torch.float32
+    X = I.reference_grid(g)
+    ins = [torch.from_numpy(X + s * (x0 - X)).to(td).pin_memory() for s in (1.0, 0.5, -0.5, 0.25, 0.0, 0.8)]
+    outs = [torch.empty_like(t).pin_memory() for t in ins]
+    sim = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype)
+    sim.set_B0(dev(B0, td))
+    for a, b in zip(ins, outs):
+        sim.step_host_async(a, b, 3, dt, op)
+    sim.host_sync()
+    ref = mr.Relaxation(g.n, g.lo, g.hi, dtype=dtype)
+    ref.set_B0(dev(B0, td))
+    for a, b in zip(ins, outs):
+        ref.set_x(a)
+        ref.step(3, dt, op)
+        want = ref.get_fields(op, x=True, host=True)["x"]
+        assert torch.equal(b, want)
+    assert sim.diagnostics(op)["steps"] == 3
+    bad = ins[0].clone().pin_memory()
+    bad[0, 0, 0, 0] += 0.1                                     # a corner node off X
+    sim.step_host_async(bad, outs[0], 1, dt, op)
+    sim.step_host_async(ins[1], outs[1], 1, dt, op)
+    with pytest.raises(mr.MrError) as e:
+        sim.host_sync()
+    assert e.value.status == mr.MR_ERR_INVALID_ARG
+    sim.step_host_async(ins[1], outs[1], 1, dt, op)            # a good state clears the failure
+    sim.host_sync()
+    fold = ins[0].clone().pin_memory()
+    fold[0, 3, 3, 3] += 5.0 * g.h[0]                           # an inner node far past its neighbours
+    sim.step_host_async(fold, outs[0], 1, dt, op)
+    with pytest.raises(mr.NumericError):
+        sim.host_sync()
+    with pytest.raises(mr.MrError):
+        sim.step(1, dt, op)                                    # failed until a new state is set
+    sim.set_x(ins[1])
+    sim.step(1, dt, op)
+
+
 def test_error_paths_on_device(mr):
     g, x0, B0, dt = case("C1")
     sim = mr.Relaxation(g.n, g.lo, g.hi)
