@@ -451,6 +451,14 @@ def test_no_write_outside_the_buffers_the_caller_gave(mr, name, bc, dtype):
             sim.get_fields_into(op, x=dense(), B=dense(), J=dense())
             sim.eps_star(g.n[0] // 2, g.n[1] // 2, 1.0, op)
     assert mr.lib.mr_get_xi(sim._ctx, C.c_void_p(dense().data_ptr())) == mr.MR_OK
+    sws = guarded(int(mr.lib.mr_stream_workspace_bytes(C.byref(gg), code)))      # the streaming host calls' staging field
+    assert mr.lib.mr_bind_stream_workspace(sim._ctx, C.c_void_p(sws.data_ptr()), sws.numel()) == mr.MR_OK
+    sim._sworkspace = sws
+    hin = torch.from_numpy(I.reference_grid(g)).to(td).pin_memory()
+    houts = [torch.empty_like(hin).pin_memory() for _ in range(3)]
+    for h in houts:
+        sim.step_host_async(hin, h, 2, dt, "mimetic")
+    sim.host_sync()
     kap = guarded(4 * g.nodes)
     nconc = C.c_int64()
     assert mr.lib.mr_convexity(sim._ctx, C.c_void_p(kap.data_ptr()), C.byref(nconc)) == mr.MR_OK
