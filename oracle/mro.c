@@ -18,7 +18,8 @@
  *   Q1  loop points I..IV are the four nearest neighbours +a, +b, -a, -b in the index surface (a,b);
  *   Q2  A = |sum_r n_r A_r| (norm of the vector sum, Eqs. 2.4/2.6/2.7);
  *   Q3  dx/dX: 2nd-order central differences inside, 2nd-order one-sided 3-point normal to a face
- *       -- parity UNPINNED against the paper (it does not state its stencil; :257 says "second-order");
+ *       -- the paper does not state its stencil (:257 says "second-order"); pinned through the whole chain only: the
+ *       relaxed states of TABLES 4.1 / 4.2 (tests/test_oracle_next.py) come out to the paper's printed digits;
  *   Q4  the "classical" operator is the analytic product/chain-rule expansion of Eq. 2.1 (:49), formulas
  *       re-derived here because Craig & Sneyd (1986) is not available -- parity UNPINNED against the paper;
  *   Q5  time stepping on this path is forward Euler with all u from the old x;
