@@ -148,6 +148,14 @@ mr_status mr_bind_stream_workspace(mr_ctx* ctx, void* workspace_dev, size_t byte
 mr_status mr_step_host_async(mr_ctx* ctx, const void* x_in_host, void* x_out_host, int64_t n, double dt, mr_operator op);
 mr_status mr_host_sync(mr_ctx* ctx);
 
+/* mr_step that also watches the run (the time series of Fig. 4.1, :245-264): n steps, and for every `every`-th of them (the
+ * first included; every = 0: none) the diagnostics of the state that step STARTS from, appended to history_host[0 .. capacity)
+ * (host memory; *written = how many).  With the mimetic operator the step kernel reduces S6 in the same pass (the diagnosis
+ * costs no memory traffic); a record equals what mr_diagnostics would return at that point, bit for bit.
+ * Synchronises like mr_step. */
+mr_status mr_step_monitored(mr_ctx* ctx, int64_t n, double dt, mr_operator op, int64_t every, mr_diag* history_host,
+                            int64_t capacity, int64_t* written);
+
 /* The velocity u = gamma J x B (Eq. 1.5, :40) of the current state, dense, context dtype, 0 on line-tied boundary
  * nodes: the right-hand side of dx/dt = u that mr_step and mr_step_adaptive integrate.  Asynchronous. */
 mr_status mr_rhs(mr_ctx* ctx, mr_operator op, void* u_dev);

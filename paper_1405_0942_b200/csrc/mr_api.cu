@@ -20,6 +20,7 @@ using namespace mr;
 namespace {
 
 constexpr int kMaxPartialBlocks = 4096;
+constexpr int kHistoryBatch = 1024;       // records of mr_step_monitored kept on the device between two copies to the host
 constexpr size_t kAlign = 256;
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -31,7 +32,7 @@ struct Layout {
     long long shift;      // element offset of the node (0, 0, 0) inside a padded field
     size_t field_bytes;   // one padded 3-component field
     size_t stage_bytes;   // one dense 3-component field
-    size_t off_xi[2], off_b, off_stage, off_partials, off_diag, off_flag, total;
+    size_t off_xi[2], off_b, off_stage, off_partials, off_history, off_diag, off_flag, total;
     size_t adaptive_total;   // the second workspace: 7 padded fields
 };
 
@@ -58,6 +59,7 @@ bool make_layout(const mr_grid* g, mr_dtype dt, const int* per, Layout* L)
     L->off_b = o; o += L->field_bytes;
     L->off_stage = o; o += L->stage_bytes;
     L->off_partials = o; o += align_up(sizeof(DiagPartial) * (2 * kMaxPartialBlocks), kAlign);
+    L->off_history = o; o += align_up(sizeof(DiagPartial) * kHistoryBatch, kAlign);
     L->off_diag = o; o += kAlign;
     L->off_flag = o; o += kAlign;
     L->total = o;
@@ -137,6 +139,7 @@ struct mr_ctx {
     void* stage() const { return ws + L.off_stage; }
     DiagPartial* partials() const { return reinterpret_cast<DiagPartial*>(ws + L.off_partials); }
     DiagPartial* diag_out() const { return reinterpret_cast<DiagPartial*>(ws + L.off_diag); }
+    DiagPartial* history() const { return reinterpret_cast<DiagPartial*>(ws + L.off_history); }
     int* flag() const { return reinterpret_cast<int*>(ws + L.off_flag); }
     double* lambda_dev() const { return reinterpret_cast<double*>(ws + L.off_flag + 8); }   // next to the flag: one memset, one copy
     double* dt_dev() const { return reinterpret_cast<double*>(ws + L.off_diag + 128); }   // the trial step length (kernels read it)
@@ -418,8 +421,9 @@ mr_status do_step(mr_ctx* c, int64_t n, double dt, mr_operator op)
     return MR_OK;
 }
 
+// S6 of the current state, enqueued: the four raw sums / extrema into *dst (device)
 template <typename T>
-mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
+mr_status enqueue_diag(mr_ctx* c, mr_operator op, DiagPartial* dst)
 {
     const long long rows = (long long)c->grid.ny * c->grid.nz;
     int blocks = c->sm_count * 8;
@@ -427,7 +431,6 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
     if (blocks > rows) blocks = (int)rows;
     const T* xi = static_cast<const T*>(c->xi(c->cur));
     const T* b = static_cast<const T*>(c->b());
-    MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
     const int threads = c->grid.nx >= 256 ? 256 : (c->grid.nx >= 128 ? 128 : (c->grid.nx >= 64 ? 64 : 32));
     const bool stream_ok = streaming(c, op);
     const StreamPlan& pl = op == MR_OP_MIMETIC ? c->plan_mim : c->plan_dir;
@@ -452,22 +455,105 @@ mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
         else k_diag<T, 1><<<blocks, threads, 0, c->stream>>>(xi, b, grid_params<T>(c), c->partials(), c->flag());
         c->launches++;
     }
-    k_diag_final<<<1, 256, 0, c->stream>>>(c->partials(), total, c->diag_out());
+    k_diag_final<<<1, 256, 0, c->stream>>>(c->partials(), total, dst);
     c->launches++;
     MR_CUDA(c, cudaGetLastError());
-    DiagPartial r;
-    MR_CUDA(c, cudaMemcpyAsync(&r, c->diag_out(), sizeof(r), cudaMemcpyDeviceToHost, c->stream));
-    int f = 0;
-    mr_status st = read_flag(c, &f);
-    if (st != MR_OK) return st;
-    const double vol8 = 8.0 * c->h[0] * c->h[1] * c->h[2];
-    out->time = c->time;
-    out->steps = c->steps;
+    return MR_OK;
+}
+
+void fill_diag(const mr_ctx* c, const DiagPartial& r, double time, int64_t steps, mr_diag* out)
+{
+    out->time = time;
+    out->steps = steps;
     out->energy = r.e / 16.0;
     out->max_jxb = r.fmax;
     out->xi = r.xi;
-    out->min_det = r.dmin / vol8;
+    out->min_det = r.dmin / (8.0 * c->h[0] * c->h[1] * c->h[2]);
+}
+
+template <typename T>
+mr_status do_diag(mr_ctx* c, mr_operator op, mr_diag* out)
+{
+    MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
+    mr_status st = enqueue_diag<T>(c, op, c->diag_out());
+    if (st != MR_OK) return st;
+    DiagPartial r;
+    MR_CUDA(c, cudaMemcpyAsync(&r, c->diag_out(), sizeof(r), cudaMemcpyDeviceToHost, c->stream));
+    int f = 0;
+    st = read_flag(c, &f);
+    if (st != MR_OK) return st;
+    fill_diag(c, r, c->time, c->steps, out);
     if (f & FLAG_NUMERIC) return fail(c, MR_ERR_NUMERIC, "mr_diagnostics: det(dx/dX) <= 0 or a non-finite value was met");
+    return MR_OK;
+}
+
+// n steps; every `every`-th of them (the first included) also reduces S6 of the state it STARTS from.  The mimetic streaming
+// kernel does both in one pass (MODE_STEPDIAG: the diagnosis costs no memory traffic); otherwise S6 is a pass of its own.  The
+// records stay on the device, kHistoryBatch at a time.
+template <typename T>
+mr_status do_step_monitored(mr_ctx* c, int64_t n, double dt, mr_operator op, int64_t every, mr_diag* hist, int64_t cap, int64_t* written)
+{
+    MR_CUDA(c, cudaMemsetAsync(c->flag(), 0, sizeof(int), c->stream));
+    const double dtg = dt * c->gamma;
+    const bool fused = op == MR_OP_MIMETIC && streaming(c, op) &&
+                       c->plan_mim.all.tiles_x * c->plan_mim.all.tiles_y * c->plan_mim.all.nchunks <= kMaxPartialBlocks;
+    static thread_local DiagPartial host[kHistoryBatch];
+    double times[kHistoryBatch];
+    int64_t stepno[kHistoryBatch];
+    int64_t total = 0;
+    int pending = 0;
+    auto flush = [&]() -> mr_status {
+        if (!pending) return MR_OK;
+        MR_CUDA(c, cudaMemcpyAsync(host, c->history(), sizeof(DiagPartial) * pending, cudaMemcpyDeviceToHost, c->stream));
+        MR_CUDA(c, cudaStreamSynchronize(c->stream));
+        for (int q = 0; q < pending; ++q) fill_diag(c, host[q], times[q], stepno[q], hist + total + q);
+        total += pending;
+        pending = 0;
+        return MR_OK;
+    };
+    const double t0 = c->time;
+    const int64_t s0 = c->steps;
+    for (int64_t s = 0; s < n; ++s) {
+        const bool rec = every > 0 && s % every == 0 && total + pending < cap;
+        if (rec) {
+            times[pending] = t0 + dt * (double)s;
+            stepno[pending] = s0 + s;
+        }
+        if (rec && fused) {
+            int nb = 0;
+            cudaError_t e = launch_sym_stepdiag<T>(c->plan_mim, c->cur, (T)dtg, c->partials(), &nb, c->flag(), c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, "streaming step + diagnostics launch", e);
+            k_diag_final<<<1, 256, 0, c->stream>>>(c->partials(), nb, c->history() + pending);
+            c->launches += 2;
+            c->variant = c->plan_mim.name;
+            wrap_ghosts<T>(c, c->xi(1 - c->cur));
+            c->cur = 1 - c->cur;
+        } else {
+            if (rec) {
+                mr_status st = enqueue_diag<T>(c, op, c->history() + pending);
+                if (st != MR_OK) return st;
+            }
+            mr_status st = launch_steps<T>(c, 1, dtg, op);
+            if (st != MR_OK) return st;
+        }
+        if (rec && ++pending == kHistoryBatch) {
+            mr_status st = flush();
+            if (st != MR_OK) return st;
+        }
+    }
+    MR_CUDA(c, cudaGetLastError());
+    mr_status st = flush();
+    if (st != MR_OK) return st;
+    c->time += dt * (double)n;
+    c->steps += n;
+    if (written) *written = total;
+    int f = 0;
+    st = read_flag(c, &f);
+    if (st != MR_OK) return st;
+    if (f & FLAG_NUMERIC) {
+        c->failed = true;
+        return fail(c, MR_ERR_NUMERIC, "mr_step_monitored: det(dx/dX) <= 0 or a non-finite value was met");
+    }
     return MR_OK;
 }
 
@@ -842,6 +928,21 @@ extern "C" mr_status mr_step(mr_ctx* ctx, int64_t n, double dt, mr_operator op)
     if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_step: B0 has not been set");
     if (ctx->failed) return fail(ctx, MR_ERR_NUMERIC, "mr_step: context is in the failed state (call mr_set_x)");
     return ctx->dtype == MR_F64 ? do_step<double>(ctx, n, dt, op) : do_step<float>(ctx, n, dt, op);
+}
+
+extern "C" mr_status mr_step_monitored(mr_ctx* ctx, int64_t n, double dt, mr_operator op, int64_t every, mr_diag* history_host,
+                                       int64_t capacity, int64_t* written)
+{
+    if (written) *written = 0;
+    if (!ctx) return MR_ERR_INVALID_ARG;
+    if (n < 0 || !(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_monitored: need n >= 0 and finite dt > 0");
+    if (every < 0 || capacity < 0 || (every > 0 && capacity > 0 && !history_host))
+        return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_monitored: need every >= 0, capacity >= 0 and a history array");
+    if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_monitored: unknown operator");
+    if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_step_monitored: B0 has not been set");
+    if (ctx->failed) return fail(ctx, MR_ERR_NUMERIC, "mr_step_monitored: context is in the failed state (call mr_set_x)");
+    return ctx->dtype == MR_F64 ? do_step_monitored<double>(ctx, n, dt, op, every, history_host, capacity, written)
+                                : do_step_monitored<float>(ctx, n, dt, op, every, history_host, capacity, written);
 }
 
 extern "C" mr_status mr_rhs(mr_ctx* ctx, mr_operator op, void* u_dev)

@@ -39,6 +39,7 @@ struct StreamArgs {
     int ox, oy, oz;       // box coordinate of the node (0, 0, 0) in the tensor maps (= the ghost widths)
     int per;              // bit a: axis a is periodic (no face, no one-sided difference, every node an inner point)
     int* flag;
+    void* partials;       // MODE_STEPDIAG: where the per-CTA partials of S6 go (the step's output is `out`)
 };
 
 // How the xy plane is cut into tiles.  `all`: every node is a tile node (what S6 needs: it sums over all of them).  `step`:
@@ -293,6 +294,7 @@ inline StreamArgs<T> stream_args(const StreamPlan& p, const Tiling& t, T dtg, in
     a.ox = p.g.ghost[0]; a.oy = p.g.ghost[1]; a.oz = p.g.ghost[2];
     a.per = (p.g.per[0] ? 1 : 0) | (p.g.per[1] ? 2 : 0) | (p.g.per[2] ? 4 : 0);
     a.flag = flag;
+    a.partials = nullptr;
     return a;
 }
 

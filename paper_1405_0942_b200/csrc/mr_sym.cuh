@@ -75,7 +75,9 @@ template <> struct Words<f2> {
 }  // namespace tmem
 inline __device__ double Lanes<double>::rcp(double d) { return fast_rcp(d); }
 
-enum : int { MODE_STEP = 0, MODE_DIAG = 1, MODE_RHS = 2 };     // xi+ = xi + dt u  |  the reduction S6  |  out = u = gamma J x B
+// xi+ = xi + dt u  |  the reduction S6  |  out = u = gamma J x B  |  the step AND S6 of the state it starts from, in one pass
+// (S6 fused into the step costs no extra HBM traffic)
+enum : int { MODE_STEP = 0, MODE_DIAG = 1, MODE_RHS = 2, MODE_STEPDIAG = 3 };
 
 // PER = false: all six faces line-tied (the hot path: no periodic logic is compiled in);  PER = true: at least one periodic axis
 template <typename T, int MODE, bool PER>
@@ -87,7 +89,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     using LN = Lanes<T>;
     using V = typename LN::V;                      // what a thread owns along i: one double, or a packed pair of floats
     using W32 = tmem::Words<V>;
-    constexpr bool DIAG = MODE == MODE_DIAG, RHS = MODE == MODE_RHS;
+    constexpr bool DIAG = MODE == MODE_DIAG || MODE == MODE_STEPDIAG, RHS = MODE == MODE_RHS, STORE = MODE != MODE_DIAG;
     constexpr int NV = L::NV;
     constexpr int TX = L::TX, TY = L::TY, NTW = L::NTW, BW = L::BW, CSX = L::CSX, CSB = L::CSB, BBW = L::BBW, BCS = L::BCS;
     constexpr int NW = L::NWARPS, WN = L::WN, C0W = L::C0W, C1W = L::C1W, REC = L::REC;
@@ -398,7 +400,8 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             cross_set(DJ, Bc, uu);
             if constexpr (DIAG) {
                 if (p > k0) diag_node(p - 1, c0, n0, Bc, uu);
-            } else {
+            }
+            if constexpr (STORE) {
                 const V s = sh[(Q + 1) & 1];
                 V x[3];
 #pragma unroll
@@ -452,7 +455,8 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
             n0[1] = W32::get(w0 + 7 * WN);
             n0[2] = W32::get(w1 + 3 * WN);
             diag_node(nz - 1, c0, n0, Bt, zero);
-        } else if (any_st) {
+        }
+        if (STORE && any_st) {
             T* pl = out + (long long)(nz - 1) * a.plane + (long long)gj * a.pitch + gi;
 #pragma unroll
             for (int c = 0; c < 3; ++c) store_nodes(pl + c * a.comp, RHS ? LN::bc(T(0)) : (ql & 1) ? xh[1][c] : xh[0][c]);
@@ -478,7 +482,7 @@ k_step_sym(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         if (tid == 0) {
             DiagPartial v = shp[0];
             for (int w = 1; w < NTW; ++w) diag_combine(v, shp[w]);
-            reinterpret_cast<DiagPartial*>(out)[blockIdx.x] = v;
+            (STORE ? static_cast<DiagPartial*>(a.partials) : reinterpret_cast<DiagPartial*>(out))[blockIdx.x] = v;
         }
     }
     if (warp == 0) tmem::dealloc<L::TMEM_COLS>(tm_base_s);
@@ -493,8 +497,11 @@ using SymKernel = void (*)(const CUtensorMap, const CUtensorMap, const T*, T*, c
 template <typename T>
 inline SymKernel<T> sym_kernel(int mode, bool per)
 {
-    if (per) return mode == MODE_STEP ? k_step_sym<T, MODE_STEP, true> : mode == MODE_DIAG ? k_step_sym<T, MODE_DIAG, true> : k_step_sym<T, MODE_RHS, true>;
-    return mode == MODE_STEP ? k_step_sym<T, MODE_STEP, false> : mode == MODE_DIAG ? k_step_sym<T, MODE_DIAG, false> : k_step_sym<T, MODE_RHS, false>;
+    if (per)
+        return mode == MODE_STEP ? k_step_sym<T, MODE_STEP, true> : mode == MODE_DIAG ? k_step_sym<T, MODE_DIAG, true>
+             : mode == MODE_RHS ? k_step_sym<T, MODE_RHS, true> : k_step_sym<T, MODE_STEPDIAG, true>;
+    return mode == MODE_STEP ? k_step_sym<T, MODE_STEP, false> : mode == MODE_DIAG ? k_step_sym<T, MODE_DIAG, false>
+         : mode == MODE_RHS ? k_step_sym<T, MODE_RHS, false> : k_step_sym<T, MODE_STEPDIAG, false>;
 }
 
 inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* xi0, void* xi1, void* b, int sm_count,
@@ -519,9 +526,9 @@ inline bool build_sym_plan(StreamPlan* p, const StreamGeom& g, bool f64, void* x
     cudaError_t e = cudaSuccess;
     const int sb = (int)p->smem_bytes;
     const bool per = g.per[0] || g.per[1] || g.per[2];
-    const void* fn[3];
-    for (int m = 0; m < 3; ++m) fn[m] = f64 ? (const void*)sym_kernel<double>(m, per) : (const void*)sym_kernel<float>(m, per);
-    for (int m = 0; m < 3 && e == cudaSuccess; ++m) e = cudaFuncSetAttribute(fn[m], cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
+    const void* fn[4];
+    for (int m = 0; m < 4; ++m) fn[m] = f64 ? (const void*)sym_kernel<double>(m, per) : (const void*)sym_kernel<float>(m, per);
+    for (int m = 0; m < 4 && e == cudaSuccess; ++m) e = cudaFuncSetAttribute(fn[m], cudaFuncAttributeMaxDynamicSharedMemorySize, sb);
     if (e != cudaSuccess) {
         *why = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e);
         return false;
@@ -549,6 +556,19 @@ inline cudaError_t launch_sym_step(const StreamPlan& p, int cur, T dtg, int* fla
     T* o = static_cast<T*>(out ? out : p.xi[1 - cur]);
     sym_kernel<T>(rhs ? MODE_RHS : MODE_STEP, a.per != 0)<<<a.ntiles * p.step.nchunks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
         p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), o, a);
+    return cudaGetLastError();
+}
+
+// One step of the state in buffer `cur` into the other state buffer AND S6 of the state it starts from: one DiagPartial per CTA
+// into `partials` (the tiling in which every node is a tile node, like launch_sym_diag: same partials, same order, same sums)
+template <typename T>
+inline cudaError_t launch_sym_stepdiag(const StreamPlan& p, int cur, T dtg, DiagPartial* partials, int* nblocks, int* flag, cudaStream_t stream)
+{
+    StreamArgs<T> a = stream_args<T>(p, p.all, dtg, flag);
+    a.partials = partials;
+    *nblocks = a.ntiles * p.all.nchunks;
+    sym_kernel<T>(MODE_STEPDIAG, a.per != 0)<<<*nblocks, SymLayout<T>::NTHREADS, p.smem_bytes, stream>>>(
+        p.map_xi[cur], p.map_b, static_cast<const T*>(p.xi[cur]), static_cast<T*>(p.xi[1 - cur]), a);
     return cudaGetLastError();
 }
 

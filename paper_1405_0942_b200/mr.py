@@ -97,6 +97,7 @@ lib.mr_launch_count.restype = C.c_int64
 lib.mr_step_variant.argtypes = [_ctx_p]
 lib.mr_step_variant.restype = C.c_char_p
 lib.mr_set_variant.argtypes = [_ctx_p, C.c_char_p]
+lib.mr_step_monitored.argtypes = [_ctx_p, C.c_int64, C.c_double, C.c_int, C.c_int64, C.POINTER(mr_diag), C.c_int64, C.POINTER(C.c_int64)]
 lib.mr_stream_workspace_bytes.argtypes = [C.POINTER(mr_grid), C.c_int]
 lib.mr_stream_workspace_bytes.restype = C.c_size_t
 lib.mr_bind_stream_workspace.argtypes = [_ctx_p, C.c_void_p, C.c_size_t]
@@ -231,6 +232,18 @@ class Relaxation:
     def step(self, n, dt, op="mimetic"):
         with self._torch.cuda.device(self.device):
             self._check(lib.mr_step(self._ctx, int(n), float(dt), _op(op)))
+
+    def step_monitored(self, n, dt, op="mimetic", every=1):
+        """mr_step_monitored: n steps; returns the diagnostics (list of dicts) of the states the steps 0, every, 2 every, ... start from."""
+        cap = 0 if every <= 0 else (int(n) + int(every) - 1) // int(every)
+        hist = (mr_diag * max(cap, 1))()
+        w = C.c_int64()
+        with self._torch.cuda.device(self.device):
+            rc = lib.mr_step_monitored(self._ctx, int(n), float(dt), _op(op), int(every), hist, cap, C.byref(w))
+        out = [{"time": h.time, "steps": h.steps, "energy": h.energy, "max_jxb": h.max_jxb, "xi": h.xi, "min_det": h.min_det}
+               for h in hist[: w.value]]
+        self._check(rc)
+        return out
 
     def diagnostics(self, op="mimetic"):
         out = mr_diag()

@@ -344,6 +344,37 @@ def test_streaming_host_calls_equal_the_synchronous_ones(mr, op, dtype):
     sim.step(1, dt, op)
 
 
+@pytest.mark.parametrize("name,bc", [("C1", None), ("pow2p1", None), ("ragged", None), ("tail1", ("line_tied", "line_tied", "periodic"))])
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_monitored_steps_equal_steps_and_diagnostics(mr, name, bc, op, dtype):
+    """mr_step_monitored: the record of step s is what mr_diagnostics returns before step s, and the state after the run is the
+    state mr_step reaches: bit for bit.  (Mimetic: the step kernel reduces S6 in the same pass, MODE_STEPDIAG; the records that
+    are not asked for cost nothing.)"""
+    g, x0, B0, dt = case(name)
+    bc = bc or ("line_tied",) * 3
+    if "periodic" in bc:
+        x0 = I.reference_grid(g)
+    a = make_sim(mr, g, x0, B0, dtype=dtype, bc=bc)
+    b = make_sim(mr, g, x0, B0, dtype=dtype, bc=bc)
+    hist = a.step_monitored(11, dt, op, every=3)               # records before the steps 0, 3, 6, 9
+    assert [h["steps"] for h in hist] == [0, 3, 6, 9]
+    for q, h in enumerate(hist):
+        d = b.diagnostics(op)
+        for k in ("energy", "max_jxb", "xi", "min_det"):
+            assert h[k] == d[k], (q, k, h[k], d[k])
+        assert h["time"] == pytest.approx(d["time"], rel=1e-14, abs=1e-300)       # (3 dt + 3 dt + ... against s dt)
+        b.step(3 if q < 3 else 2, dt, op)
+    assert torch.equal(a.get_xi(), b.get_xi())
+    da, db = a.diagnostics(op), b.diagnostics(op)
+    assert all(da[k] == db[k] for k in ("steps", "energy", "max_jxb", "xi", "min_det"))
+    assert a.step_monitored(5, dt, op, every=0) == []          # no records asked for: plain steps
+    b.step(5, dt, op)
+    assert torch.equal(a.get_xi(), b.get_xi())
+    one = a.step_monitored(1, dt, op, every=1)
+    assert len(one) == 1 and one[0]["steps"] == 16
+
+
 def test_error_paths_on_device(mr):
     g, x0, B0, dt = case("C1")
     sim = mr.Relaxation(g.n, g.lo, g.hi)
