@@ -200,6 +200,40 @@ mr_status mr_eps_star(mr_ctx* ctx, mr_operator op, int32_t ic, int32_t jc, doubl
  * the references are dense device arrays in the context dtype (for the IsoHelix field Eqs. 3.3 and 3.2). */
 mr_status mr_sigma(mr_ctx* ctx, const void* x_ref_dev, const void* B_ref_dev, double* sigma_x, double* sigma_B);
 
+/* ---- the one entry point that needs no device memory beyond its input and output ------------------------------------
+ * Everything above works in a workspace the caller allocates.  Some callers cannot allocate at all: a plug-in that runs
+ * inside a host application whose own memory manager has taken the whole card (a raw cudaMalloc there fails, or fights the
+ * pool), a monitoring hook in a time-critical loop (cudaMalloc and cudaFree stall every stream of the device while they
+ * run), or code that is simply handed two pointers and a stream and nothing else.  For them: the convexity check of
+ * Eqs. 3.10-3.11 (:231-243, the early warning of :333) on a dense array of node POSITIONS, without a context.  The call
+ * issues no cudaMalloc, cudaFree, or library routine that allocates; its only scratch memory is a fixed array of
+ * MR_NOALLOC_MAX_PLANES 64-bit counters (8 KiB) built into libmr.so, which every GPU that loads the library carries until
+ * the process ends.
+ *
+ *   x_dev      in   T[3][nz][ny][nx] positions (dense, i fastest), T by `dtype`; device memory of the current device
+ *   grid       in   2 <= nx, ny <= 4096, 2 <= nz <= MR_NOALLOC_MAX_PLANES.  A grid with more z-planes than the scratch has
+ *                   counters for is refused with MR_ERR_INVALID_ARG before anything is launched (mr_last_error(NULL) says so);
+ *                   such a grid needs mr_convexity on a context.
+ *   kappa_dev  out  int32[nz][ny][nx], +1 / -1 per node as mr_convexity writes it; may be NULL
+ *   n_concave  out  host: how many nodes have kappa = -1
+ *   stream          cudaStream_t of the caller (0 = legacy default stream); the call waits for it before it returns
+ *
+ * All six faces are treated as ends of the grid (a node there has only the trihedra whose neighbours exist), which is what
+ * mr_convexity does on a context without periodic axes; the two then agree node for node -- up to trihedra whose determinant
+ * is within rounding of zero, because this call differences the positions while a context differences the displacements it
+ * stores (in fp64 a 1e-14 effect).
+ *
+ * Set-up: the FIRST call on each device looks up where the built-in array lives on that device (and thereby loads the
+ * library's kernels there); make that first call outside any stream capture.  Later calls on the device reuse the address.
+ * Sharing: there is ONE array per device, used by every call from every thread, and it keeps what the last call counted.
+ * Each call zeroes the counters it is going to use (on `stream`) before its kernel runs, so calls that follow one another
+ * on the GPU are independent; two calls that can overlap on the GPU (different streams, or different threads without
+ * ordering between their streams) race on the counters and return garbage counts -- serialise them.
+ * Errors go to mr_last_error(NULL), like those of mr_create. */
+#define MR_NOALLOC_MAX_PLANES 1024
+mr_status mr_convexity_noalloc(const void* x_dev, const mr_grid* grid, mr_dtype dtype, int32_t* kappa_dev, int64_t* n_concave,
+                               void* stream);
+
 /* Message for the last error on this context ("" if none); ctx == NULL gives the last mr_create failure.
  * The pointer stays valid until the next failing call on the same context (or mr_destroy). */
 const char* mr_last_error(const mr_ctx* ctx);

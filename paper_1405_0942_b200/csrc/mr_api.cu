@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -1195,5 +1196,125 @@ extern "C" mr_status mr_set_variant(mr_ctx* ctx, const char* name)
     else if (!std::strcmp(name, "graph")) ctx->graphs_enabled = true;        // (the default) mr_step replays CUDA graphs on small grids
     else if (!std::strcmp(name, "nograph")) ctx->graphs_enabled = false;
     else return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_variant: expected auto, generic, graph or nograph");
+    return MR_OK;
+}
+
+// ------------------------------------------------------------------------------- mr_convexity_noalloc (include/mr.h)
+// Convexity of a dense array of node positions for callers that have no way to hand the library device memory beyond their
+// own input and output: the per-plane counters the kernel needs live in this file-scope array, which is part of the loaded
+// module (MR_NOALLOC_MAX_PLANES * 8 bytes = 8 KiB on every GPU that loads libmr.so, until the process exits).
+//
+// In host code `g_noalloc_counts` is only a handle for the runtime, not a device address, so it is never passed to a kernel:
+// noalloc_scratch() asks the runtime once per device (with that device current) where the array lives there and the launch
+// gets that pointer.
+
+static __device__ __align__(256) unsigned long long g_noalloc_counts[MR_NOALLOC_MAX_PLANES];
+
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+unsigned long long* g_noalloc_ptr[kNoallocMaxDevices];      // device address of g_noalloc_counts per device ordinal, null = not asked yet
+
+// the array's address on the current device (first use on a device: cudaGetSymbolAddress, which also loads the module there)
+cudaError_t noalloc_scratch(unsigned long long** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kNoallocMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_counts);
+        if (e != cudaSuccess) return e;
+        g_noalloc_ptr[dev] = static_cast<unsigned long long*>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return cudaSuccess;
+}
+
+// k_convexity (mr_next.cuh) on dense positions x[3][nz][ny][nx], every face an open end of the grid: kappa = +1 iff each
+// trihedron of the node whose three neighbours exist has sgn det = di dj dk (Eqs. 3.10-3.11).  The nodes
+// with kappa = -1 are counted per z-plane into plane_count[k] (zeroed by the caller): one atomic per block that found any.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_convexity_dense(const T* __restrict__ x, int nx, int ny, int nz, int* __restrict__ kappa, unsigned long long* __restrict__ plane_count)
+{
+    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k = blockIdx.z;
+    const bool in = i < nx && j < ny;
+    const long long N = (long long)nx * ny * nz, p = ((long long)k * ny + j) * nx + i;
+    int kap = 1;
+    if (in) {
+        const int idx[3] = { i, j, k }, n[3] = { nx, ny, nz };
+        const long long stride[3] = { 1, nx, (long long)nx * ny };
+        double e[3][2][3];      // edge vectors to the six neighbours (doubles: their sign decides an integer)
+        bool have[3][2];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                have[a][s] = s == 0 ? idx[a] > 0 : idx[a] < n[a] - 1;
+                const long long o = s == 0 ? -stride[a] : stride[a];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) e[a][s][c] = have[a][s] ? (double)x[c * N + p + o] - (double)x[c * N + p] : 0.0;
+            }
+#pragma unroll
+        for (int si = 0; si < 2; ++si)
+#pragma unroll
+            for (int sj = 0; sj < 2; ++sj)
+#pragma unroll
+                for (int sk = 0; sk < 2; ++sk) {
+                    if (!(have[0][si] && have[1][sj] && have[2][sk])) continue;
+                    const double* u = e[0][si];
+                    const double* v = e[1][sj];
+                    const double* w = e[2][sk];
+                    const double d = u[0] * (v[1] * w[2] - v[2] * w[1]) - u[1] * (v[0] * w[2] - v[2] * w[0]) + u[2] * (v[0] * w[1] - v[1] * w[0]);
+                    const int sgn = d > 0.0 ? 1 : (d < 0.0 ? -1 : 0);
+                    const int prod = (si ? 1 : -1) * (sj ? 1 : -1) * (sk ? 1 : -1);
+                    if (sgn != prod) kap = -1;
+                }
+        if (kappa) kappa[p] = kap;
+    }
+    __shared__ int sh[8];
+    const unsigned concave = __ballot_sync(0xffffffffu, in && kap < 0);
+    if (threadIdx.x == 0) sh[threadIdx.y] = __popc(concave);
+    __syncthreads();
+    if (threadIdx.x == 0 && threadIdx.y == 0) {
+        int total = 0;
+        for (int w = 0; w < 8; ++w) total += sh[w];
+        if (total) atomicAdd(plane_count + k, (unsigned long long)total);
+    }
+}
+
+}  // namespace
+
+extern "C" mr_status mr_convexity_noalloc(const void* x_dev, const mr_grid* grid, mr_dtype dtype, int32_t* kappa_dev, int64_t* n_concave,
+                                          void* stream)
+{
+    if (!x_dev || !grid || !n_concave) return fail(nullptr, MR_ERR_INVALID_ARG, "mr_convexity_noalloc: null argument");
+    if (dtype != MR_F64 && dtype != MR_F32) return fail(nullptr, MR_ERR_INVALID_ARG, "mr_convexity_noalloc: dtype must be MR_F64 or MR_F32");
+    if (grid->nx < 2 || grid->ny < 2 || grid->nz < 2 || grid->nx > 4096 || grid->ny > 4096)
+        return fail(nullptr, MR_ERR_INVALID_ARG, "mr_convexity_noalloc: need 2 <= nx, ny <= 4096 and nz >= 2");
+    if (grid->nz > MR_NOALLOC_MAX_PLANES)
+        return fail(nullptr, MR_ERR_INVALID_ARG,
+                    "mr_convexity_noalloc: nz = " + std::to_string(grid->nz) + " is more than the " + std::to_string(MR_NOALLOC_MAX_PLANES) +
+                        " z-planes the library's static scratch has counters for (MR_NOALLOC_MAX_PLANES); use mr_convexity on a context instead");
+    unsigned long long* counts = nullptr;
+    MR_CUDA(nullptr, noalloc_scratch(&counts));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int nz = grid->nz;
+    // the array still holds whatever the previous call (of any thread, on this device) counted
+    MR_CUDA(nullptr, cudaMemsetAsync(counts, 0, sizeof(unsigned long long) * nz, s));
+    const dim3 block(32, 8, 1), blocks((grid->nx + 31) / 32, (grid->ny + 7) / 8, nz);
+    if (dtype == MR_F64) k_convexity_dense<double><<<blocks, block, 0, s>>>(static_cast<const double*>(x_dev), grid->nx, grid->ny, nz, kappa_dev, counts);
+    else k_convexity_dense<float><<<blocks, block, 0, s>>>(static_cast<const float*>(x_dev), grid->nx, grid->ny, nz, kappa_dev, counts);
+    MR_CUDA(nullptr, cudaGetLastError());
+    unsigned long long host[MR_NOALLOC_MAX_PLANES];
+    MR_CUDA(nullptr, cudaMemcpyAsync(host, counts, sizeof(unsigned long long) * nz, cudaMemcpyDeviceToHost, s));
+    MR_CUDA(nullptr, cudaStreamSynchronize(s));
+    unsigned long long total = 0;
+    for (int k = 0; k < nz; ++k) total += host[k];
+    *n_concave = (int64_t)total;
     return MR_OK;
 }

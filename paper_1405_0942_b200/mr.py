@@ -104,6 +104,9 @@ lib.mr_bind_stream_workspace.argtypes = [_ctx_p, C.c_void_p, C.c_size_t]
 lib.mr_step_host_async.argtypes = [_ctx_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int]
 lib.mr_host_sync.argtypes = [_ctx_p]
 lib.mr_set_variant.restype = C.c_int
+lib.mr_convexity_noalloc.argtypes = [C.c_void_p, C.POINTER(mr_grid), C.c_int, C.c_void_p, C.POINTER(C.c_int64), C.c_void_p]
+lib.mr_convexity_noalloc.restype = C.c_int
+NOALLOC_MAX_PLANES = 1024      # MR_NOALLOC_MAX_PLANES of include/mr.h
 
 
 class MrError(RuntimeError):
@@ -129,6 +132,34 @@ def workspace_bytes(n, dtype="f64", bc=("line_tied",) * 3) -> int:
 
 def _op(op):
     return OPERATORS[op] if isinstance(op, str) else int(op)
+
+
+def convexity_noalloc(x, kappa=None):
+    """mr_convexity_noalloc: how many nodes of the position field ``x`` are concave (Eq. 3.11), with no context and no
+    workspace.  It is the call for code that may not allocate on the GPU (a plug-in inside an application that owns all
+    device memory, a check inside a loop that cannot afford the device-wide stall of cudaMalloc): the library allocates
+    nothing, and neither does this wrapper -- the only scratch is a small array built into ``libmr.so``.
+
+    ``x``: contiguous CUDA tensor (3, nz, ny, nx), float64 or float32, with nz <= ``NOALLOC_MAX_PLANES`` (more planes raise
+    ``MrError``; use ``Relaxation.convexity``).  ``kappa``: optional int32 CUDA tensor (nz, ny, nx) OF THE CALLER'S that
+    receives +1 / -1 per node.  Runs on the current stream of ``x``'s device and waits for it.  All calls on a device share
+    that one scratch array: do not issue calls that can overlap on the GPU (other streams, other threads)."""
+    import torch
+
+    if x.device.type != "cuda" or x.dtype not in (torch.float64, torch.float32) or x.dim() != 4 or x.shape[0] != 3 or not x.is_contiguous():
+        raise MrError(MR_ERR_INVALID_ARG, "x must be a contiguous float64/float32 CUDA tensor of shape (3, nz, ny, nx)")
+    nz, ny, nx = (int(v) for v in x.shape[1:])
+    if kappa is not None and (kappa.device != x.device or kappa.dtype != torch.int32 or tuple(kappa.shape) != (nz, ny, nx)
+                              or not kappa.is_contiguous()):
+        raise MrError(MR_ERR_INVALID_ARG, "kappa must be a contiguous int32 tensor of shape (nz, ny, nx) on x's device")
+    n = C.c_int64()
+    with torch.cuda.device(x.device):
+        st = lib.mr_convexity_noalloc(x.data_ptr(), C.byref(mr_grid(nx, ny, nz)), MR_F64 if x.dtype == torch.float64 else MR_F32,
+                                      kappa.data_ptr() if kappa is not None else None, C.byref(n),
+                                      torch.cuda.current_stream(x.device).cuda_stream)
+    if st != MR_OK:
+        _raise(st, None)
+    return int(n.value)
 
 
 class Relaxation:
