@@ -235,6 +235,13 @@ class Relaxation:
             self.stream.wait_stream(cur)
             t.record_stream(self.stream)
 
+    def _publish(self):
+        """The other direction of _order, after an asynchronous call that writes (or still reads) a caller tensor on the library's
+        stream: the caller's current stream waits for it, so the caller may use the tensor there without synchronising."""
+        cur = self._torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            cur.wait_stream(self.stream)
+
     def _host(self, t, name):
         if t is None:
             return None
@@ -252,6 +259,7 @@ class Relaxation:
                 self._check(lib.mr_set_B0_host(self._ctx, self._host(B0, "B0")))
             else:
                 self._check(lib.mr_set_B0(self._ctx, self._dev(B0, "B0")))
+                self._publish()
 
     def set_x(self, x):
         with self._torch.cuda.device(self.device):
@@ -300,6 +308,7 @@ class Relaxation:
                 self._check(lib.mr_get_fields_host(self._ctx, _op(op), self._host(x, "x"), self._host(B, "B"), self._host(J, "J")))
             else:
                 self._check(lib.mr_get_fields(self._ctx, _op(op), self._dev(x, "x"), self._dev(B, "B"), self._dev(J, "J")))
+                self._publish()
 
     def set_xi(self, xi):
         """mr_set_xi: the displacement x - X (what fp32 contexts should exchange instead of positions)."""
@@ -310,6 +319,7 @@ class Relaxation:
         out = self.empty_field()
         with self._torch.cuda.device(self.device):
             self._check(lib.mr_get_xi(self._ctx, self._dev(out, "xi")))
+            self._publish()
         return out
 
     def rhs(self, op="mimetic"):
@@ -317,6 +327,7 @@ class Relaxation:
         out = self.empty_field()
         with self._torch.cuda.device(self.device):
             self._check(lib.mr_rhs(self._ctx, _op(op), self._dev(out, "u")))
+            self._publish()
         return out
 
     def step_adaptive(self, t_end, lambda0, dt, op="mimetic", max_trials=1000000, trace=False):

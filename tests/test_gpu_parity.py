@@ -541,6 +541,86 @@ def test_full_size_config4_direct_operator_matches_oracle(mr):
         assert d[k] == pytest.approx(o[k], rel=TOL_STEP), k
 
 
+@pytest.mark.parametrize("op", ["mimetic", "direct"])
+def test_full_size_config2_100_steps_both_operators(mr, op):
+    """BASELINE configs[1] on its OWN grid (64x64x192, both operators side by side), SURVEY 8(d)'s 100-step gate: this is the
+    grid on which mr_step replays CUDA graphs over 2x4 tiles and several z-chunks, so the graph and the plain-launch variant
+    are both held against the oracle: x <= 1e-9, the displacement moved to 1e-7, S6 of the state reached to 1e-8."""
+    cfg = I.CONFIGS["C2"]
+    g = cfg.grid
+    assert g.n == (64, 64, 192)
+    x0, B0, dt = I.make(cfg)
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 100, op=opcode(op))
+    o = mro.diagnostics(g.n, g.lo, g.hi, ref, B0, op=opcode(op))
+    moved = np.abs(ref - x0).max()
+    assert moved > 0
+    xs = {}
+    for v in ("graph", "nograph"):
+        sim = make_sim(mr, g, x0, B0)
+        sim.set_variant(v)
+        sim.step(100, dt, op)
+        assert sim.step_variant == ("sym_tmem_f64" if op == "mimetic" else "direct_tma_f64"), sim.step_variant
+        xs[v] = sim.get_fields(x=True)["x"].cpu().numpy()
+        assert nrel(xs[v], ref) < TOL_100
+        assert np.abs(xs[v] - ref).max() < 1e-7 * moved
+        d = sim.diagnostics(op)
+        assert d["steps"] == 100
+        for k in ("energy", "max_jxb", "xi", "min_det"):
+            assert d[k] == pytest.approx(o[k], rel=1e-8), (v, k)
+    assert np.array_equal(xs["graph"], xs["nograph"])
+
+
+def test_full_size_config4_20_step_prefix_matches_oracle(mr):
+    """BASELINE configs[3] (256x256x512) through a 20-step prefix of its run, from the configuration's own initial state, in
+    the launch configuration bench.py times: x to 1e-9 and to 1e-7 of the distance moved, S6 of the state reached to 1e-8
+    (the oracle needs about half a minute with all host threads)."""
+    cfg = I.CONFIGS["C4"]
+    g = cfg.grid
+    x0, B0, dt = I.make(cfg)
+    sim = make_sim(mr, g, x0, B0)
+    sim.step(20, dt)
+    assert sim.step_variant == "sym_tmem_f64"
+    x20 = sim.get_fields(x=True, host=True)["x"].numpy()
+    d = sim.diagnostics()
+    del sim
+    ref = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 20)
+    moved = np.abs(ref - x0).max()
+    assert moved > 0
+    assert nrel(x20, ref) < TOL_100
+    assert np.abs(x20 - ref).max() < 1e-7 * moved
+    o = mro.diagnostics(g.n, g.lo, g.hi, ref, B0)
+    for k in ("energy", "max_jxb", "xi", "min_det"):
+        assert d[k] == pytest.approx(o[k], rel=1e-8), k
+
+
+def test_context_on_a_side_stream_hands_its_results_to_the_callers_stream(mr):
+    """A context bound to a stream other than the caller's current one: mr_get_fields, mr_get_xi and mr_rhs are asynchronous on
+    the context's stream, so the binding makes the caller's stream wait for them; the tensors are used at once on the
+    current stream (no synchronisation in between) and must equal those of a context on the current stream."""
+    cfg = I.scaled(I.CONFIGS["C3"], (128, 128, 128))
+    g = cfg.grid
+    x0, B0, dt = I.make(cfg)
+    td = torch.float64
+    side = torch.cuda.Stream()
+    want = make_sim(mr, g, x0, B0)
+    want.step(3, dt)
+    got = mr.Relaxation(g.n, g.lo, g.hi, stream=side)
+    got.set_B0(dev(B0, td))
+    if not np.array_equal(x0, I.reference_grid(g)):
+        got.set_x(dev(x0, td))
+    got.step(3, dt)
+    assert got.stream == side and torch.cuda.current_stream() != side
+    for op in ("mimetic", "direct"):
+        a = got.get_xi().clone()
+        b = got.rhs(op).clone()
+        f = {k: v.clone() for k, v in got.get_fields(op, x=True, B=True, J=True).items()}
+        assert torch.equal(a, want.get_xi())
+        assert torch.equal(b, want.rhs(op))
+        w = want.get_fields(op, x=True, B=True, J=True)
+        for k in ("x", "B", "J"):
+            assert torch.equal(f[k], w[k]), (op, k)
+
+
 def test_fp32_context_accepts_the_fp32_rounding_of_the_reference_grid(mr):
     """mr_set_x on an fp32 context: boundary nodes given as float32(X) are on the reference grid (|X|/h is large
     on config 5: 4 / (8/511)), one really displaced boundary node is still refused."""
