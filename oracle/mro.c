@@ -31,7 +31,10 @@
  *   Q22 integrator (section 2.4, :131-143): Cash-Karp RK5(4), the step advances with the fifth-order solution,
  *       Lambda = max over nodes and components of |x5 - x4|; reject if Lambda > Lambda0 and retry with Eq. 2.11;
  *       accept otherwise, and enlarge dt by Eq. 2.11 if Lambda < Lambda0/2 (growth capped at 5x: Lambda may be 0);
- *       the last step is clipped to end at t_end without changing the dt handed on;
+ *       the last step is clipped to end at t_end without changing the dt handed on; a recomputation uses at most 0.9 dt;
+ *   Q26 a trial in which a stage folds the grid (det <= 0 or non-finite) is rejected and recomputed with dt/2; 40 such
+ *       trials in a row stop the run (:333 "a drop of the time step by several orders of magnitude, at which point the
+ *       simulation is stopped");
  *   Q23 convexity (Eqs. 3.10-3.11, :231-243): kappa(node) = 1 iff every trihedron of the node whose three
  *       neighbours exist has sgn det = di dj dk, else -1;
  *   Q24 eps* (Eq. 3.7, :214): alpha* = J.B/B^2 at the interior nodes of the grid line through (i_c, j_c), maximum
@@ -595,25 +598,42 @@ int mro_cash_karp_trial(long long m, const double* y, double dt, mro_rhs_fn f, v
     return MRO_OK;
 }
 
-/*
- * Step control of PAPER.md:139-143: returns 1 if the trial step is accepted (Lambda <= Lambda0), 0 if it is
- * rejected, and writes the step length to use next: Eq. 2.11 dt' = dt |Lambda0/Lambda|^0.2 after a rejection or
- * when Lambda < Lambda0/2 (growth capped at 5 dt, Lambda may vanish), dt otherwise.  A retry after a rejection is at
- * most 0.9 dt (reading Q22): Eq. 2.11 alone has a fixed point just above Lambda0, where the factor rounds to 1
- * and the same trial would be repeated for ever (met on the IsoHelix run of Table 4.1: Lambda = 1.0000000000000002e-8).
- */
-int mro_step_control(double dt, double lambda, double lambda0, double* dt_next)
+/* Eq. 2.11: dt' = dt |Lambda0 / Lambda|^0.2 */
+static double eq_2_11(double dt, double Lambda, double Lambda0)
 {
-    if (lambda > lambda0 || isnan(lambda)) {
-        const double f = isnan(lambda) ? 0.5 : pow(fabs(lambda0 / lambda), 0.2);
-        *dt_next = dt * (f < 0.9 ? f : 0.9);
+    return dt * pow(fabs(Lambda0 / Lambda), 0.2);
+}
+
+/*
+ * The step control as section 2.4 words it, sentence by sentence.  Returns 1 if the result of the
+ * trial is kept, 0 if it "is rejected and recomputed with dt = dt'"; *dt_prime is the step length to go on with.
+ * Three guards are not in the paper's text; each is a separate clause below and a reading in DESIGN.md:
+ *   Q22a  a recomputation is tried with at most 0.9 dt: just above Lambda0 the factor of Eq. 2.11 rounds to 1 and the very
+ *         same trial would be recomputed for ever (met at Lambda = 1.0000000000000002e-8, Lambda0 = 1e-8 on the IsoHelix
+ *         run of TABLE 4.1); 0.9 is the safety factor of the stepper the paper cites for its error measure ([21]);
+ *   Q22b  an increase is at most 5 dt: Lambda may be 0 (a state at rest), where Eq. 2.11 has no value;
+ *   Q26   a trial without an error measure (Lambda is NaN) is treated like one that folded the grid: recomputed with dt/2.
+ */
+int mro_step_control(double dt, double Lambda, double Lambda0, double* dt_prime)
+{
+    if (isnan(Lambda)) {                        /* Q26 */
+        *dt_prime = 0.5 * dt;
         return 0;
     }
-    if (lambda < 0.5 * lambda0) {
-        double f = lambda > 0.0 ? pow(fabs(lambda0 / lambda), 0.2) : 5.0;
-        *dt_next = dt * (f > 5.0 ? 5.0 : f);
-    } else {
-        *dt_next = dt;
+    /* "If the error in x exceeds a prescribed limit the step length is reduced via (2.11) ... If Lambda > Lambda0 the
+     * result is rejected and recomputed with dt = dt'." */
+    if (Lambda > Lambda0) {
+        *dt_prime = eq_2_11(dt, Lambda, Lambda0);
+        if (*dt_prime > 0.9 * dt) *dt_prime = 0.9 * dt;          /* Q22a */
+        return 0;
+    }
+    /* the result is kept; the step length stays ... */
+    *dt_prime = dt;
+    /* ... unless: "Should Lambda fall below Lambda0/2, dt' is increased according to the same equation" */
+    if (Lambda < Lambda0 / 2.0) {
+        const double most = 5.0 * dt;                             /* Q22b */
+        *dt_prime = Lambda > 0.0 ? eq_2_11(dt, Lambda, Lambda0) : most;
+        if (*dt_prime > most) *dt_prime = most;
     }
     return 1;
 }
@@ -628,11 +648,19 @@ static int relax_rhs(const double* x, double* u, void* user)
     return mro_fields(r->n, r->lo, r->hi, x, r->B0, r->gamma, r->op, NULL, NULL, u, NULL);
 }
 
+/* how many trials in a row may fold the grid before the run is given up (reading Q26): 2^-40 = 9e-13, "a drop of the
+ * time step by several orders of magnitude, at which point the simulation is stopped" */
+#define MRO_MAX_FOLDED_TRIALS 40
+
 /*
- * Integrate dx/dt = u(x) = gamma J x B (Eq. 1.5) from *t to t_end with the adaptive Cash-Karp scheme.
+ * Integrate dx/dt = u(x) = gamma J x B (Eq. 1.5) from *t to t_end with the adaptive Cash-Karp scheme of section 2.4.
  * *dt: first trial step in, step handed on out.  trace (may be NULL, capacity trace_cap rows of 4 doubles) records every
- * trial: {t, dt tried, Lambda, accepted}.  counts[0] = accepted, counts[1] = rejected trials.
- * Returns 0, 1 (bad argument), 5 (numeric failure; x holds the last accepted state) or 7 (max_trials exhausted).
+ * trial: {t, dt tried, Lambda, kept}.  counts[0] = results kept, counts[1] = results rejected.
+ *
+ * A trial in which some stage meets det(dx/dX) <= 0 or a non-finite value has no result at all; the paper does not say
+ * what its code does then (reading Q26): it counts as rejected (Lambda = NaN in the trace) and is recomputed with half the
+ * step; MRO_MAX_FOLDED_TRIALS of them in a row end the run with return code 5, x being the last kept state (:333).
+ * Returns 0, 1 (bad argument), 5 (numeric failure as just described) or 7 (max_trials exhausted).
  */
 int mro_step_adaptive(const int n[3], const double lo[3], const double hi[3], double* x, const double* B0, double gamma,
                       int op, double t_end, double lambda0, double* t, double* dt, long long max_trials,
@@ -643,32 +671,46 @@ int mro_step_adaptive(const int n[3], const double lo[3], const double hi[3], do
     const long long m = (long long)(3 * g.N);
     double* work = (double*)malloc((size_t)8 * (size_t)m * sizeof(double));
     if (!work) return MRO_BADARG;
-    double* y5 = work + (size_t)7 * (size_t)m;
+    double* x_new = work + (size_t)7 * (size_t)m;
     relax_rhs_t r = { n, lo, hi, B0, gamma, op };
     counts[0] = counts[1] = 0;
     long long trials = 0;
+    int folded_in_a_row = 0;
     rc = MRO_OK;
-    while (*t < t_end) {
+    while (*t < t_end && rc == MRO_OK) {
         if (trials >= max_trials) { rc = 7; break; }
-        const double rest = t_end - *t;
-        const int clipped = *dt >= rest;
-        const double h = clipped ? rest : *dt;
-        double lam = 0.0, dt_next = 0.0;
-        rc = mro_cash_karp_trial(m, x, h, relax_rhs, &r, y5, NULL, &lam, work);
-        if (rc) break;
-        const int ok = mro_step_control(h, lam, lambda0, &dt_next);
+        /* the step to try: dt, or what is left to t_end if that is shorter (the run ends exactly there) */
+        const double left = t_end - *t;
+        const int is_last = *dt >= left;
+        const double tried = is_last ? left : *dt;
+        double Lambda = NAN, dt_prime = 0.0;
+        int kept = 0;
+        const int trial_rc = mro_cash_karp_trial(m, x, tried, relax_rhs, &r, x_new, NULL, &Lambda, work);
+        if (trial_rc == MRO_NUMERIC) {
+            /* Q26: no result; recompute with half the step, give up after MRO_MAX_FOLDED_TRIALS in a row */
+            Lambda = NAN;
+            dt_prime = 0.5 * tried;
+            if (++folded_in_a_row >= MRO_MAX_FOLDED_TRIALS) rc = MRO_NUMERIC;
+        } else if (trial_rc != MRO_OK) {
+            rc = trial_rc;
+            break;
+        } else {
+            folded_in_a_row = 0;
+            kept = mro_step_control(tried, Lambda, lambda0, &dt_prime);
+        }
         if (trace && trials < trace_cap) {
-            trace[4 * trials + 0] = *t; trace[4 * trials + 1] = h; trace[4 * trials + 2] = lam; trace[4 * trials + 3] = (double)ok;
+            double* row = trace + 4 * trials;
+            row[0] = *t; row[1] = tried; row[2] = Lambda; row[3] = (double)kept;
         }
         ++trials;
-        if (ok) {
-            memcpy(x, y5, (size_t)m * sizeof(double));
-            *t = clipped ? t_end : *t + h;
-            counts[0]++;
-            if (!clipped || dt_next < *dt) *dt = dt_next;      /* a clipped last step does not change the dt handed on */
+        counts[kept ? 0 : 1]++;
+        if (kept) {
+            memcpy(x, x_new, (size_t)m * sizeof(double));
+            *t = is_last ? t_end : *t + tried;
+            /* the shortened last step says nothing about the step length: hand on the caller's dt unless the control shrank it */
+            if (!is_last || dt_prime < *dt) *dt = dt_prime;
         } else {
-            counts[1]++;
-            *dt = dt_next;
+            *dt = dt_prime;                   /* "recomputed with dt = dt'" */
         }
     }
     free(work);

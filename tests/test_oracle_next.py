@@ -83,6 +83,44 @@ def test_step_control_follows_the_paper():
     assert not ok and dtn == pytest.approx(0.1 * 0.5 ** 0.2, rel=1e-14)   # 0.871 < 0.9: Eq. 2.11 as printed
 
 
+def test_a_trial_that_folds_the_grid_is_recomputed_with_half_the_step():
+    """Reading Q26 (the paper only says the run "is stopped" after "a drop of the time step by several orders of magnitude",
+    PAPER.md:333): a step far beyond the stability limit turns cells inside out in a stage; such a trial has no result, is
+    rejected with Lambda = NaN and recomputed with dt/2 until a stage survives.  It leaves no trace in x: the run equals, bit
+    for bit, one that starts with the first step length that did not fold."""
+    cfg = I.CONFIGS["C1"]
+    g = cfg.grid
+    x0, B0, _ = I.make(cfg)
+    x, t, dt_next, (acc, rej), trace = mro.step_adaptive(g.n, g.lo, g.hi, x0, B0, t_end=1.0, lam0=1e-7, dt=4.0)
+    folded = np.isnan(trace[:, 2])
+    nf = int(folded.sum())
+    assert nf >= 2 and folded[:nf].all() and not folded[nf:].any()            # they come first, in a row
+    assert np.array_equal(trace[:nf, 1], 1.0 * 0.5 ** np.arange(nf))          # 4.0 is clipped to t_end = 1, then halved
+    assert not trace[:nf, 3].any() and np.all(trace[:nf, 0] == 0.0)
+    assert trace[nf, 1] == 0.5 ** nf and t == 1.0 and acc + rej == len(trace) and rej >= nf
+    x2, t2, dt2, (acc2, rej2), trace2 = mro.step_adaptive(g.n, g.lo, g.hi, x0, B0, t_end=1.0, lam0=1e-7, dt=0.5 ** nf)
+    assert np.array_equal(x, x2) and dt2 == dt_next and acc2 == acc and rej2 == rej - nf
+    assert np.array_equal(trace2, trace[nf:])
+
+
+def test_forty_folded_trials_in_a_row_stop_the_run():
+    """Reading Q26, the other half: a state that is folded already (one node pushed past its third neighbour) fails in the first
+    stage whatever the step; after 40 halvings (2^-40 = 9e-13 of the first step: "several orders of magnitude") the run
+    stops with the numeric return code, the state untouched."""
+    cfg = I.CONFIGS["C1"]
+    g = cfg.grid
+    x0, B0, _ = I.make(cfg)
+    xf = x0.copy()
+    xf[0, 9, 5, 5] = x0[0, 9, 5, 8]                 # x_6 - x_4 ... fine, but x_7 - x_5 < 0: det(dx/dX) < 0 at node 6
+    assert mro.diagnostics(g.n, g.lo, g.hi, xf, B0, strict=False)["min_det"] < 0
+    with pytest.raises(mro.NumericError):
+        mro.step_adaptive(g.n, g.lo, g.hi, xf, B0, t_end=1.0, lam0=1e-7, dt=0.125)
+    x, t, dt_next, (acc, rej), trace = mro.step_adaptive(g.n, g.lo, g.hi, xf, B0, t_end=1.0, lam0=1e-7, dt=0.125, strict=False)
+    assert (acc, rej) == (0, 40) and t == 0.0 and np.array_equal(x, xf)
+    assert dt_next == 0.125 * 0.5 ** 40 and np.isnan(trace[:, 2]).all()
+    assert np.array_equal(trace[:, 1], 0.125 * 0.5 ** np.arange(40))
+
+
 def test_adaptive_relaxation_on_config1():
     """C1 with the adaptive integrator: the run ends exactly at t_end, rejected trials leave no trace in x, every
     accepted Lambda is within tolerance, the energy decays monotonically over the accepted steps,
