@@ -142,7 +142,10 @@ mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_host, void* B_
  * mr_stream_workspace_bytes = 3 nx ny nz elements).  x_in_host / x_out_host: [3][nz][ny][nx] in the context dtype, pinned host
  * memory (pageable memory works but serialises the copies); both must stay valid and x_out_host unread until mr_host_sync.
  * mr_host_sync waits for everything enqueued and reports what mr_set_x / mr_step would have: MR_ERR_INVALID_ARG if some
- * x_in had a line-tied boundary node off the reference grid, MR_ERR_NUMERIC if some state folded (the context is then failed). */
+ * x_in had a line-tied boundary node off the reference grid, MR_ERR_NUMERIC if some state folded (the context is then failed).
+ * Between the first mr_step_host_async and mr_host_sync the error word of the context belongs to the calls in flight: the
+ * calls that use it themselves (mr_set_x, mr_set_x_host, mr_set_xi, mr_step, mr_step_monitored, mr_step_adaptive,
+ * mr_diagnostics, mr_eps_star, mr_get_fields_host) return MR_ERR_STATE until mr_host_sync has been called. */
 size_t mr_stream_workspace_bytes(const mr_grid* grid, mr_dtype dtype);
 mr_status mr_bind_stream_workspace(mr_ctx* ctx, void* workspace_dev, size_t bytes);
 mr_status mr_step_host_async(mr_ctx* ctx, const void* x_in_host, void* x_out_host, int64_t n, double dt, mr_operator op);
@@ -179,9 +182,12 @@ typedef struct {
  * and brings ONE scalar back; the host rejects the trial if Lambda > lambda0 and retries with dt' = dt |lambda0/Lambda|^0.2
  * (Eq. 2.11), accepts it otherwise and enlarges dt by the same formula if Lambda < lambda0/2 (growth capped at 5x).
  * The last step is clipped to end at t_end.  *dt: first trial step in, step handed on out.  trace_host (may be NULL):
- * trace_cap rows {t, dt tried, Lambda, accepted} of the trials.  Returns MR_ERR_STATE without B0 or without the
- * adaptive workspace, MR_ERR_NUMERIC if a stage met det <= 0 (the state is then the last accepted one),
- * MR_ERR_INVALID_ARG if max_trials ran out before t_end. */
+ * trace_cap rows {t, dt tried, Lambda, accepted} of the trials.  A trial in which a stage met det <= 0 or a non-finite value
+ * has no result: it counts as rejected (Lambda = NaN in the trace) and is retried with dt/2 (reading Q26; the
+ * paper reports "a drop of the time step by several orders of magnitude, at which point the simulation is stopped", :333).
+ * Returns MR_ERR_STATE without B0 or without the adaptive workspace; MR_ERR_NUMERIC after 40 such trials in a row (2^-40
+ * of the step first tried), or if the step length underflows: the state is then the last accepted one, *dt the collapsed
+ * step; MR_ERR_INVALID_ARG if max_trials ran out before t_end. */
 mr_status mr_step_adaptive(mr_ctx* ctx, double t_end, double lambda0, double* dt, mr_operator op, int64_t max_trials,
                            mr_adapt_stats* stats, double* trace_host, int64_t trace_cap);
 

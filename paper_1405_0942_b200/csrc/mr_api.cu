@@ -515,6 +515,9 @@ mr_status do_step_monitored(mr_ctx* c, int64_t n, double dt, mr_operator op, int
     const double t0 = c->time;
     const int64_t s0 = c->steps;
     for (int64_t s = 0; s < n; ++s) {
+        // (the clock follows the state: an early return below leaves time / steps at the step the state has reached)
+        c->time = t0 + dt * (double)s;
+        c->steps = s0 + s;
         const bool rec = every > 0 && s % every == 0 && total + pending < cap;
         if (rec) {
             times[pending] = t0 + dt * (double)s;
@@ -542,11 +545,11 @@ mr_status do_step_monitored(mr_ctx* c, int64_t n, double dt, mr_operator op, int
             if (st != MR_OK) return st;
         }
     }
+    c->time = t0 + dt * (double)n;
+    c->steps = s0 + n;
     MR_CUDA(c, cudaGetLastError());
     mr_status st = flush();
     if (st != MR_OK) return st;
-    c->time += dt * (double)n;
-    c->steps += n;
     if (written) *written = total;
     int f = 0;
     st = read_flag(c, &f);
@@ -650,6 +653,8 @@ mr_status rk_trial(mr_ctx* c, mr_operator op, double h, double* lambda, int* num
     return MR_OK;
 }
 
+constexpr int kMaxFoldedTrials = 40;     // trials in a row that may fold the grid (each retried at dt/2) before the run is given up
+
 // Eq. 2.11 and the accept / reject rule of PAPER.md:139-143 (reading Q22)
 bool step_control(double dt, double lambda, double lambda0, double* dt_next)
 {
@@ -674,6 +679,7 @@ mr_status do_adaptive(mr_ctx* c, double t_end, double lambda0, double* dt, mr_op
 {
     mr_adapt_stats s = { 0, 0, 0, c->time, *dt, 0.0 };
     int64_t trials = 0;
+    int folded_in_a_row = 0;            // DESIGN.md reading Q26
     mr_status rc = MR_OK;
     while (c->time < t_end) {
         if (trials >= max_trials) { rc = fail(c, MR_ERR_INVALID_ARG, "mr_step_adaptive: max_trials exhausted before t_end"); break; }
@@ -685,7 +691,8 @@ mr_status do_adaptive(mr_ctx* c, double t_end, double lambda0, double* dt, mr_op
         rc = rk_trial<T>(c, op, h, &lam, &numeric);
         if (rc != MR_OK) break;
         s.rhs_evals += 6;
-        if (numeric & FLAG_NUMERIC) lam = NAN;           // a stage folded the grid: the trial counts as failed
+        if (numeric & FLAG_NUMERIC) { lam = NAN; ++folded_in_a_row; }   // a stage folded the grid: the trial counts as failed
+        else folded_in_a_row = 0;
         s.last_lambda = lam;
         const bool ok = step_control(h, lam, lambda0, &dt_next);
         if (trace && trials < trace_cap) {
@@ -701,7 +708,10 @@ mr_status do_adaptive(mr_ctx* c, double t_end, double lambda0, double* dt, mr_op
         } else {
             s.rejected++;
             *dt = dt_next;
-            if (!(dt_next > 1e-300)) { rc = fail(c, MR_ERR_NUMERIC, "mr_step_adaptive: the step length collapsed (cf. PAPER.md:333)"); break; }
+            if (folded_in_a_row >= kMaxFoldedTrials || !(dt_next > 1e-300)) {
+                rc = fail(c, MR_ERR_NUMERIC, "mr_step_adaptive: the step length collapsed (cf. PAPER.md:333)");
+                break;
+            }
         }
     }
     s.time = c->time;
@@ -887,6 +897,7 @@ extern "C" mr_status mr_set_B0_host(mr_ctx* ctx, const void* B0_host)
 extern "C" mr_status mr_set_x(mr_ctx* ctx, const void* x_dev)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_set_x: mr_step_host_async calls are in flight (mr_host_sync first)");
     if (!x_dev) return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_x: null pointer");
     return ctx->dtype == MR_F64 ? do_set_x<double>(ctx, x_dev, false) : do_set_x<float>(ctx, x_dev, false);
 }
@@ -895,6 +906,7 @@ extern "C" mr_status mr_set_x_host(mr_ctx* ctx, const void* x_host)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
     if (!x_host) return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_x_host: null pointer");
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_set_x_host: mr_step_host_async calls are in flight (mr_host_sync first)");
     MR_CUDA(ctx, cudaMemcpyAsync(ctx->stage(), x_host, ctx->dense_bytes(), cudaMemcpyHostToDevice, ctx->stream));
     return mr_set_x(ctx, ctx->stage());
 }
@@ -902,6 +914,7 @@ extern "C" mr_status mr_set_x_host(mr_ctx* ctx, const void* x_host)
 extern "C" mr_status mr_set_xi(mr_ctx* ctx, const void* xi_dev)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_set_xi: mr_step_host_async calls are in flight (mr_host_sync first)");
     if (!xi_dev) return fail(ctx, MR_ERR_INVALID_ARG, "mr_set_xi: null pointer");
     return ctx->dtype == MR_F64 ? do_set_x<double>(ctx, xi_dev, true) : do_set_x<float>(ctx, xi_dev, true);
 }
@@ -924,6 +937,7 @@ extern "C" mr_status mr_get_xi(mr_ctx* ctx, void* xi_dev)
 extern "C" mr_status mr_step(mr_ctx* ctx, int64_t n, double dt, mr_operator op)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_step: mr_step_host_async calls are in flight (mr_host_sync first)");
     if (n < 0 || !(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step: need n >= 0 and finite dt > 0");
     if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step: unknown operator");
     if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_step: B0 has not been set");
@@ -936,6 +950,7 @@ extern "C" mr_status mr_step_monitored(mr_ctx* ctx, int64_t n, double dt, mr_ope
 {
     if (written) *written = 0;
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_step_monitored: mr_step_host_async calls are in flight (mr_host_sync first)");
     if (n < 0 || !(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_monitored: need n >= 0 and finite dt > 0");
     if (every < 0 || capacity < 0 || (every > 0 && capacity > 0 && !history_host))
         return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_monitored: need every >= 0, capacity >= 0 and a history array");
@@ -991,6 +1006,7 @@ extern "C" mr_status mr_step_adaptive(mr_ctx* ctx, double t_end, double lambda0,
                                       mr_adapt_stats* stats, double* trace_host, int64_t trace_cap)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_step_adaptive: mr_step_host_async calls are in flight (mr_host_sync first)");
     if (!dt || !(*dt > 0.0) || !std::isfinite(*dt) || !(lambda0 > 0.0) || !std::isfinite(t_end) || max_trials < 0)
         return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_adaptive: need finite t_end, lambda0 > 0, *dt > 0, max_trials >= 0");
     if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_step_adaptive: unknown operator");
@@ -1004,6 +1020,7 @@ extern "C" mr_status mr_step_adaptive(mr_ctx* ctx, double t_end, double lambda0,
 extern "C" mr_status mr_diagnostics(mr_ctx* ctx, mr_operator op, mr_diag* out)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_diagnostics: mr_step_host_async calls are in flight (mr_host_sync first)");
     if (!out) return fail(ctx, MR_ERR_INVALID_ARG, "mr_diagnostics: null output");
     if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_diagnostics: unknown operator");
     if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_diagnostics: B0 has not been set");
@@ -1034,6 +1051,7 @@ extern "C" mr_status mr_convexity(mr_ctx* ctx, int32_t* kappa_dev, int64_t* n_co
 extern "C" mr_status mr_eps_star(mr_ctx* ctx, mr_operator op, int32_t ic, int32_t jc, double a_r, double* alpha_host, double* eps_star)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_eps_star: mr_step_host_async calls are in flight (mr_host_sync first)");
     if (!eps_star) return fail(ctx, MR_ERR_INVALID_ARG, "mr_eps_star: null output");
     if (op != MR_OP_MIMETIC && op != MR_OP_DIRECT) return fail(ctx, MR_ERR_INVALID_ARG, "mr_eps_star: unknown operator");
     if (!ctx->have_B0) return fail(ctx, MR_ERR_STATE, "mr_eps_star: B0 has not been set");
@@ -1066,6 +1084,7 @@ extern "C" mr_status mr_get_fields(mr_ctx* ctx, mr_operator op, void* x_dev, voi
 extern "C" mr_status mr_get_fields_host(mr_ctx* ctx, mr_operator op, void* x_host, void* B_host, void* J_host)
 {
     if (!ctx) return MR_ERR_INVALID_ARG;
+    if (ctx->pipeline_open) return fail(ctx, MR_ERR_STATE, "mr_get_fields_host: mr_step_host_async calls are in flight (mr_host_sync first)");
     void* outs[3] = { x_host, B_host, J_host };
     MR_CUDA(ctx, cudaMemsetAsync(ctx->flag(), 0, sizeof(int), ctx->stream));
     for (int w = 0; w < 3; ++w) {

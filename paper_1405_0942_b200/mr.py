@@ -408,11 +408,17 @@ class Relaxation:
                     self._sworkspace = torch.empty(nb, dtype=torch.uint8, device=self.device)
                 self._check(lib.mr_bind_stream_workspace(self._ctx, self._sworkspace.data_ptr(), nb))
             self._check(lib.mr_step_host_async(self._ctx, self._host(x_in, "x_in"), self._host(x_out, "x_out"), int(n), float(dt), _op(op)))
+            # the copies are queued, not done: hold both host tensors until host_sync() (a pinned block dropped by the caller
+            # could be handed out again by the host allocator while a copy still uses it)
+            self.__dict__.setdefault("_in_flight", []).append((x_in, x_out))
 
     def host_sync(self):
         """mr_host_sync: wait for every step_host_async enqueued; raises what mr_set_x / mr_step would have raised."""
-        with self._torch.cuda.device(self.device):
-            self._check(lib.mr_host_sync(self._ctx))
+        try:
+            with self._torch.cuda.device(self.device):
+                self._check(lib.mr_host_sync(self._ctx))
+        finally:
+            self.__dict__.get("_in_flight", []).clear()
 
     def close(self):
         if getattr(self, "_ctx", None):

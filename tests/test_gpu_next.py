@@ -411,6 +411,41 @@ def test_pontin09_phi_pi_breaks_down_after_the_grid_turns_concave(mr):
     assert st["time"] == 200.0 and eps > 0.3 and direct.diagnostics("direct")["xi"] < 1e-3
 
 
+def test_folding_trials_follow_the_oracle(mr):
+    """Reading Q26 on both sides (section 2.4 is silent): a trial in which a stage folds the grid is rejected with
+    Lambda = NaN and retried at dt/2 -- same trace as the oracle through the folded trials and the recovery -- and a state that
+    is folded already ends the run after 40 such trials with the numeric code, the state and the clock untouched."""
+    cfg = I.CONFIGS["C1"]
+    g = cfg.grid
+    x0, B0, _ = I.make(cfg)
+    sim = make_sim(mr, g, x0, B0)
+    st = sim.step_adaptive(t_end=1.0, lambda0=1e-7, dt=4.0, trace=True)
+    xr, t, dtn, (acc, rej), trace = mro.step_adaptive(g.n, g.lo, g.hi, x0, B0, t_end=1.0, lam0=1e-7, dt=4.0)
+    tr = np.array(st["trace"])
+    nf = int(np.isnan(trace[:, 2]).sum())
+    assert nf >= 2 and (st["accepted"], st["rejected"]) == (acc, rej) and st["time"] == t == 1.0
+    assert np.array_equal(np.isnan(tr[:, 2]), np.isnan(trace[:, 2]))
+    assert np.array_equal(tr[:nf, [0, 1, 3]], trace[:nf, [0, 1, 3]])                    # the folded trials: bit for bit
+    assert np.array_equal(tr[:, 3], trace[:, 3])
+    assert np.allclose(tr[nf:, 1], trace[nf:, 1], rtol=1e-6, atol=0) and np.allclose(tr[nf:, 2], trace[nf:, 2], rtol=1e-5, atol=0)
+    assert nrel(sim.get_fields(x=True)["x"].cpu().numpy(), xr) < 1e-9
+    assert st["dt_next"] == pytest.approx(dtn, rel=1e-6)
+    # a state that is folded from the start (one inner node pushed past its third neighbour)
+    xf = x0.copy()
+    xf[0, 9, 5, 5] = x0[0, 9, 5, 8]
+    sim.set_x(dev(xf))
+    before = sim.get_xi().clone()
+    with pytest.raises(mr.NumericError):
+        sim.step_adaptive(t_end=1.0, lambda0=1e-7, dt=0.125, trace=True)
+    la = sim.last_adaptive
+    _, t, dtn, (acc, rej), trace = mro.step_adaptive(g.n, g.lo, g.hi, xf, B0, t_end=1.0, lam0=1e-7, dt=0.125, strict=False)
+    assert (la["accepted"], la["rejected"]) == (acc, rej) == (0, 40) and la["time"] == t == 0.0
+    assert la["dt_next"] == dtn == 0.125 * 0.5 ** 40
+    tr = np.array(la["trace"])
+    assert np.isnan(tr[:, 2]).all() and np.array_equal(tr[:, [0, 1, 3]], trace[:, [0, 1, 3]])
+    assert torch.equal(sim.get_xi(), before)
+
+
 def test_isohelix_relaxation_on_the_gpu_follows_the_oracle(mr):
     """The same run at n = 17 on both sides to t = 64 (the oracle's Lambda is |x5 - x4|, the library's the weighted stage sum:
     the two agree to ~1e-7, so near Lambda0 a trial may be judged differently and the step sequences part; the states they

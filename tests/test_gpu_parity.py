@@ -324,6 +324,15 @@ def test_streaming_host_calls_equal_the_synchronous_ones(mr, op, dtype):
         want = ref.get_fields(op, x=True, host=True)["x"]
         assert torch.equal(b, want)
     assert sim.diagnostics(op)["steps"] == 3
+    # while calls are in flight the error word belongs to them: the calls that use it are refused until the sync
+    sim.step_host_async(ins[0], outs[0], 1, dt, op)
+    for call in (lambda: sim.step(1, dt, op), lambda: sim.diagnostics(op), lambda: sim.set_x(ins[1]), lambda: sim.set_x(dev(x0, td)),
+                 lambda: sim.get_fields(op, x=True, host=True), lambda: sim.step_monitored(2, dt, op)):
+        with pytest.raises(mr.MrError) as e:
+            call()
+        assert e.value.status == mr.MR_ERR_STATE
+    sim.host_sync()
+    assert sim.diagnostics(op)["steps"] == 1
     bad = ins[0].clone().pin_memory()
     bad[0, 0, 0, 0] += 0.1                                     # a corner node off X
     sim.step_host_async(bad, outs[0], 1, dt, op)
