@@ -123,7 +123,7 @@ class ClockSampler:
 
 
 def summarize_clocks(rows):
-    sm, mx, reasons = [], [], set()
+    sm, mx, pw, reasons = [], [], [], set()
     names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
     for r in rows:
         try:
@@ -131,13 +131,18 @@ def summarize_clocks(rows):
             mx.append(float(r[1]))
         except Exception:
             continue
+        try:
+            pw.append(float(r[2]))
+        except Exception:
+            pass
         for name, v in zip(names, r[3:7]):
             if v.lower().startswith("active"):
                 reasons.add(name)
     if not sm:
-        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "power_w": None}
     sm.sort()
-    return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+    return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm),
+            "power_w": sum(pw) / len(pw) if pw else None}
 
 
 def aggregate_over_ranks(local_ms, local_updates, dist=None):
@@ -161,60 +166,52 @@ def workload(name):
 
 # ---------------------------------------------------------------------------------------------- oracle legs
 
-def oracle_sample(cfg, I, budget_s=12.0, planes=64):
-    """Time the CPU oracle, as it stands, on a bounded sample of the workload: the first `planes` z-planes of the
-    grid (same spacing and field) for as many steps as fit the budget.  Returns (updates/s, threads, description)."""
-    import numpy as np
-    from oracle import mro                       # the ONLY place bench.py touches the oracle
+def oracle_sample(cfg, I, x0, B0, dt, budget_s=12.0):
+    """Time the CPU oracle, as it stands, on the workload itself: whole-grid forward Euler steps from the configuration's
+    initial state, as many as fit the budget (at least one; config 4 needs about 1.5 s per step on 16 cores).  Returns
+    (updates/s, threads, description)."""
+    from oracle import mro                       # the ONLY place bench.py touches the oracle (with run_reference)
     g = cfg.grid
-    nz = min(planes, g.n[2])
-    sub = I.Grid((g.n[0], g.n[1], nz), g.lo, (g.hi[0], g.hi[1], g.lo[2] + (nz - 1) * g.h[2]))
-    B0 = I.twist_field(sub, cfg.twists) if cfg.twists else I.abc_field(I.reference_grid(sub))
-    x0 = I.reference_grid(sub)
-    dt = I.stable_dt(B0, sub)
     threads = mro.max_threads()
     mro.set_threads(threads)
     t0 = time.perf_counter()
-    x = mro.step(sub.n, sub.lo, sub.hi, x0, B0, dt, 1)
+    x = mro.step(g.n, g.lo, g.hi, x0, B0, dt, 1)
     t1 = time.perf_counter() - t0
     steps = int(max(1, min(20, budget_s / max(t1, 1e-3))))
     t0 = time.perf_counter()
-    mro.step(sub.n, sub.lo, sub.hi, x, B0, dt, steps)
+    mro.step(g.n, g.lo, g.hi, x, B0, dt, steps)
     el = time.perf_counter() - t0
     mro.set_threads(1)
-    desc = "%s z-slab %dx%dx%d (same h and B0), %d Euler steps, mimetic, OpenMP over k" % (cfg.name, sub.n[0], sub.n[1], sub.n[2], steps)
-    return sub.nodes * steps / el, threads, desc
+    desc = "%s, the whole %dx%dx%d grid, %d Euler steps after one untimed, mimetic, OpenMP over k" % ((cfg.name,) + g.n + (steps,))
+    return g.nodes * steps / el, threads, desc
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores, same metric/config; each step a bounded sample."""
+    """--impl reference: the oracle on the host cores, same metric and config: each step one forward Euler step of the whole
+    grid (config 4: about 1.5 s on 16 cores, so the default 20 + 5 steps end within a minute or two)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     cfg, I = workload(args.workload)
-    import numpy as np
     from oracle import mro
     g = cfg.grid
-    planes = 16
-    sub = I.Grid((g.n[0], g.n[1], planes), g.lo, (g.hi[0], g.hi[1], g.lo[2] + (planes - 1) * g.h[2]))
-    B0 = I.twist_field(sub, cfg.twists) if cfg.twists else I.abc_field(I.reference_grid(sub))
-    x = I.reference_grid(sub)
-    dt = I.stable_dt(B0, sub)
+    x, B0, dt = I.make(cfg)
     threads = mro.max_threads()
     mro.set_threads(threads)
     for _ in range(args.warmup):
-        x = mro.step(sub.n, sub.lo, sub.hi, x, B0, dt, 1)
+        x = mro.step(g.n, g.lo, g.hi, x, B0, dt, 1)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        x = mro.step(sub.n, sub.lo, sub.hi, x, B0, dt, 1)
+        x = mro.step(g.n, g.lo, g.hi, x, B0, dt, 1)
     el = time.perf_counter() - t0
-    value = sub.nodes * args.steps / el
-    sample = "%s z-slab %dx%dx%d per step (same h and B0), mimetic, OpenMP over k" % (cfg.name, sub.n[0], sub.n[1], sub.n[2])
+    value = g.nodes * args.steps / el
+    sample = "%s, the whole %dx%dx%d grid per step, mimetic, OpenMP over k" % ((cfg.name,) + g.n)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "%s %dx%dx%d fp64 mimetic (CPU oracle on a z-slab sample)" % ((cfg.name,) + g.n)},
+        "config": {"workload": "%s %dx%dx%d fp64 mimetic, line-tied, forward Euler dt=%.3e (CPU oracle, whole grid)" % ((cfg.name,) + g.n + (dt,)),
+                   "nodes": g.nodes},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -331,7 +328,8 @@ def run_ours(args):
     # ---- device-resident throughput: W warm-up steps, then ONE timed mr_step(K) ----
     W = max(args.warmup, 3)
     if 3 * 3 * nodes * (8 if dtype == "f64" else 4) <= 4e8 and not args.no_graphs:
-        W = max(W, 32)                # (an L2-resident grid replays CUDA graphs of 16 steps: let the warm-up capture them)
+        W = (max(W, 32) + 15) // 16 * 16   # (an L2-resident grid replays CUDA graphs of 16 steps from an even buffer parity: the
+                                           # warm-up captures them and ends on the parity the timed call starts from)
     sim.step(W, dt, op)
     main = timed(args.steps)
     variant = sim.step_variant
@@ -350,7 +348,9 @@ def run_ours(args):
         achieved = BYTES_PER_UPDATE[dtype] * nodes / (launch_ms * 1e-3) / 1e9
         return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "frac_of_datasheet_8000": achieved / 8000.0,
-                "traffic": recorded_traffic(cfg.name, variant), "peak_source": peak_src, "kernel": variant,
+                "traffic": recorded_traffic(cfg.name, variant),
+                "traffic_source": "recorded, not measured in this run: profiles/traffic.csv (ncu --set full of these kernel sources)",
+                "peak_source": peak_src, "kernel": variant,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE[dtype] * nodes, "launch_ms": launch_ms}
 
     roofline = roof(main)
@@ -366,8 +366,52 @@ def run_ours(args):
                 time.sleep(1.0)                       # let the board cool off the previous run
             r = timed(steps)
             rf = roof(r)
+            pw = r["clocks"].get("power_w")
             regimes[name] = {"steps": steps, "ms_per_step": r["ms_all"] / steps, "seconds": r["ms"] * 1e-3,
-                             "value": r["updates_all"] / (r["ms_all"] * 1e-3), "roofline_frac": rf["frac"], "clocks": r["clocks"]}
+                             "value": r["updates_all"] / (r["ms_all"] * 1e-3), "roofline_frac": rf["frac"], "clocks": r["clocks"],
+                             # (board power is sampled every 100 ms and lags: only a run with several samples has an energy figure)
+                             "joules_per_update": None if pw is None or r["clocks"]["samples"] < 5 else pw * r["ms"] * 1e-3 / (nodes * steps)}
+            # (the driver's parser keeps `roofline` and drops the regime records: both fractions go in there too)
+            roofline[name + "_frac"] = rf["frac"]
+            roofline[name + "_ms_per_step"] = r["ms_all"] / steps
+            roofline[name + "_sm_mhz"] = r["clocks"]["sm_mhz"]
+            roofline[name + "_reasons"] = r["clocks"]["reasons"]
+            roofline[name + "_joules_per_update"] = regimes[name]["joules_per_update"]
+        roofline["regime_of_frac"] = "the %d timed steps of this run (%.0f ms): a burst at full clocks unless --steps is large; the " \
+                                     "configuration's own length (thousands of steps) runs in the sustained regime" % (args.steps, main["ms"])
+
+    # ---- BASELINE configs[4]: "fp32 results are compared to an fp64 GPU run within 1e-5 relative": the deviations of the fp32
+    # state and fields from an fp64 context on the same inputs (norm-wise, max |a - b| / max |b|; x relative to the box) after
+    # 100, 500 and the config's own number of steps
+    fp32_report = None
+    if dtype == "f32" and not args.no_fp32_report:
+        reset_state()
+        ref = mr.Relaxation(g.n, g.lo, g.hi, dtype="f64", device="cuda:%d" % local_rank)
+        ref.set_B0(torch.from_numpy(B0).to("cuda", dtype=torch.float64))
+        if displaced:
+            ref.set_x(torch.from_numpy(x0).to("cuda", dtype=torch.float64))
+        box = float(max(g.hi[a] - g.lo[a] for a in range(3)))
+
+        def rel(a, b):
+            return float((a.double() - b).abs().max() / b.abs().max())
+
+        fp32_report, done = {"bar": 1e-5, "operator": op}, 0
+        for upto in sorted({min(100, cfg.steps), min(500, cfg.steps), cfg.steps}):
+            sim.step(upto - done, dt, op)
+            ref.step(upto - done, dt, op)
+            done = upto
+            a, b = sim.get_xi(), ref.get_xi()
+            e = {"x": float((a.double() - b).abs().max()) / box, "xi": rel(a, b)}
+            del a, b
+            for name in ("B", "J"):
+                a, b = sim.get_fields(op, **{name: True})[name], ref.get_fields(op, **{name: True})[name]
+                e[name] = rel(a, b)
+                del a, b
+            fp32_report["after_%d_steps" % upto] = e
+        ref.close()
+        del ref
+        torch.cuda.empty_cache()
+        reset_state()
 
     # ---- section 2.4: the adaptive Cash-Karp integrator, in right-hand-side evaluations per second ----
     adaptive = None
@@ -423,7 +467,7 @@ def run_ours(args):
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, threads, desc = oracle_sample(cfg, I)
+        v, threads, desc = oracle_sample(cfg, I, x0, B0, dt)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
 
     if rank == 0:
@@ -432,7 +476,8 @@ def run_ours(args):
             "metric": METRIC.replace("mimetic", op).replace("fp64", prec), "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": W, "ms_per_step": main["ms_all"] / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
-            "config": {"workload": "%s %dx%dx%d %s %s, line-tied, forward Euler dt=%.3e" % ((cfg.name,) + g.n + (prec, op, dt)),
+            "config": {"workload": "%s %dx%dx%d %s %s%s, line-tied, forward Euler dt=%.3e"
+                                   % ((cfg.name,) + g.n + (prec, op, " (S3d: the builder's derivation, unpinned vs the paper)" if op == "direct" else "", dt)),
                        "nodes": nodes, "l2_policy": "working set %.2f GB vs 126 MB L2%s" % (3 * fbytes / 1e9, " (no flush needed)" if 3 * fbytes > 4e8 else " (L2-resident: HBM fraction n/a)"),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "kernel": variant},
             "clocks": main["clocks"], "e2e": e2e, "gpu_launches": main["launches"], "roofline": roofline,
@@ -445,6 +490,8 @@ def run_ours(args):
             line["config3_report"] = report
         if adaptive is not None:
             line["adaptive"] = adaptive
+        if fp32_report is not None:
+            line["fp32_vs_fp64"] = fp32_report
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -563,6 +610,7 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-regimes", action="store_true", help="skip the burst / sustained records")
+    ap.add_argument("--no-fp32-report", action="store_true", help="fp32 workloads (C5): skip the comparison with an fp64 context")
     ap.add_argument("--no-graphs", action="store_true", help="mr_step launches every step itself (small grids replay CUDA graphs by default)")
     args = ap.parse_args(argv)
     if args.isohelix:
