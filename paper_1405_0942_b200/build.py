@@ -38,8 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("MR_NVCC_EXTRA", "").split()      # e.g. -DMR_... for kernel experiments
-    cmd = [nvcc] + NVCC_FLAGS + extra + ["-I", INCLUDE, "-o", LIB] + sources()
+    cmd = [nvcc] + NVCC_FLAGS + ["-I", INCLUDE, "-o", LIB] + sources()
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         print(res.stdout)

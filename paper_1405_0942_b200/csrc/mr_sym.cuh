@@ -56,11 +56,7 @@ struct SymLayout {
     static constexpr size_t BYTES = OFF_BAR + (size_t)NB * 8 + 128;
     // TMEM record of a node: chunk 0 = columns 0, 1 of dF, n_0[0], n_0[1] (8 values), chunk 1 = column 2 of dF, n_0[2]
     static constexpr int WN = (int)sizeof(typename Lanes<T>::V) / 4;     // 32-bit words per value (a double or a pair of floats)
-    #ifdef MR_X_TMEM
-    static constexpr int C0W = 8 * WN, C1W = 8 * WN, REC = 16 * WN; // + own xi (3 values) in chunk 1
-#else
     static constexpr int C0W = 8 * WN, C1W = 4 * WN, REC = 16 * WN; // record stride (12 values, padded to 16)
-#endif
     static constexpr int TMEM_COLS = (NTW / 4) * 2 * REC;           // warps of a lane quarter x two records (plane parity)
 };
 

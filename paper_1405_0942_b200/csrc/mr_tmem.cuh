@@ -95,39 +95,6 @@ template <int N> __device__ __forceinline__ void ld(uint32_t taddr, uint32_t (&r
     if constexpr (N == 16) ld16(taddr, r); else if constexpr (N == 8) ld8(taddr, r); else ld4(taddr, r);
 }
 
-// One value per operation: a double is its own aligned register pair, so that no register has to be moved into a
-// contiguous block (the x16 forms cost ~2 moves per value); measured ~2.5 clk per operation and scheduler.
-__device__ __forceinline__ void st1(uint32_t taddr, double v)
-{
-    asm volatile("{\n\t.reg .b32 lo, hi;\n\tmov.b64 {lo, hi}, %1;\n\ttcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {lo, hi};\n\t}" ::"r"(taddr), "d"(v));
-}
-__device__ __forceinline__ void st1(uint32_t taddr, float v)
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(__float_as_uint(v)));
-}
-__device__ __forceinline__ void ld1(uint32_t taddr, double& v)
-{
-    asm volatile("{\n\t.reg .b32 lo, hi;\n\ttcgen05.ld.sync.aligned.32x32b.x2.b32 {lo, hi}, [%1];\n\tmov.b64 %0, {lo, hi};\n\t}" : "=d"(v) : "r"(taddr));
-}
-__device__ __forceinline__ void ld1(uint32_t taddr, float& v)
-{
-    uint32_t w;
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(w) : "r"(taddr));
-    v = __uint_as_float(w);
-}
-// wait for every earlier tcgen05.ld of this thread; the 16 values pass through as in/out operands (see wait_ld above)
-__device__ __forceinline__ void wait_ld_vals(double (&v)[16])
-{
-    asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+d"(v[0]), "+d"(v[1]), "+d"(v[2]), "+d"(v[3]), "+d"(v[4]), "+d"(v[5]), "+d"(v[6]), "+d"(v[7]), "+d"(v[8]),
-                   "+d"(v[9]), "+d"(v[10]), "+d"(v[11]), "+d"(v[12]), "+d"(v[13]), "+d"(v[14]), "+d"(v[15]));
-}
-__device__ __forceinline__ void wait_ld_vals(float (&v)[16])
-{
-    asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]), "+f"(v[8]),
-                   "+f"(v[9]), "+f"(v[10]), "+f"(v[11]), "+f"(v[12]), "+f"(v[13]), "+f"(v[14]), "+f"(v[15]));
-}
 __device__ __forceinline__ void wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // value <-> 32-bit words (a double is a register pair: no instruction is spent on the conversion)

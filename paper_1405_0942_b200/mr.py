@@ -10,7 +10,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MR_LIB") or os.path.join(_HERE, "libmr.so")     # MR_LIB: another build of the same ABI (A/B timing)
+LIB_PATH = os.path.join(_HERE, "libmr.so")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(
