@@ -249,6 +249,13 @@ const char* mr_last_error(const mr_ctx* ctx);
 int64_t mr_launch_count(const mr_ctx* ctx);
 const char* mr_step_variant(const mr_ctx* ctx);
 
+/* Measurement aid for the roofline of the direct operator, which is bound by plain FP64 arithmetic (bench.py --operator
+ * direct): runs a kernel of independent DFMA chains (8 per thread, no memory traffic; 8 CTAs of 256 threads per SM) back to
+ * back on `stream` for about `seconds` (0 < seconds <= 60), times it with CUDA events and writes the rate in TFLOP/s (2 FLOP
+ * per DFMA) to *tflops: a short run gives the burst figure at full clocks, a run of seconds the one under the board's power
+ * cap.  Needs no context; allocates no device memory; waits for the stream.  Errors go to mr_last_error(NULL). */
+mr_status mr_measure_fp64_peak(double seconds, void* stream, double* tflops);
+
 /* Choose the step kernel.  "auto" (default): the streaming TMA kernels (mimetic: csrc/mr_sym.cuh, direct:
  * csrc/mr_direct.cuh).  "generic": the global-memory kernels of csrc/mr_generic.cuh for both operators (one thread per
  * node, every stencil value straight from global memory): the A/B reference of the tests.  Both agree to rounding.

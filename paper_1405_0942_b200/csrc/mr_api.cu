@@ -1337,3 +1337,67 @@ extern "C" mr_status mr_convexity_noalloc(const void* x_dev, const mr_grid* grid
     *n_concave = (int64_t)total;
     return MR_OK;
 }
+
+// ------------------------------------------------------------------------------- mr_measure_fp64_peak (include/mr.h)
+// The roof of the direct operator is plain FP64 arithmetic: a kernel of independent DFMA chains, no memory
+// traffic, timed with CUDA events, gives the rate the FP64 pipes of this board deliver in the regime asked for.
+static __device__ double g_fp64_sink;
+
+namespace {
+constexpr int kPeakChains = 8, kPeakIters = 4096;
+
+__global__ void __launch_bounds__(256) k_fp64_chains(double seed)
+{
+    double a[kPeakChains];
+#pragma unroll
+    for (int c = 0; c < kPeakChains; ++c) a[c] = seed + (double)(threadIdx.x + c);
+    const double m = 1.0 - 1e-9 * seed, b = 1e-9;
+#pragma unroll 4
+    for (int it = 0; it < kPeakIters; ++it)
+#pragma unroll
+        for (int c = 0; c < kPeakChains; ++c) a[c] = fma(a[c], m, b);
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < kPeakChains; ++c) s += a[c];
+    if (s == -1.0) g_fp64_sink = s;          // never true: keeps the chains alive
+}
+}  // namespace
+
+extern "C" mr_status mr_measure_fp64_peak(double seconds, void* stream, double* tflops)
+{
+    if (!tflops || !(seconds > 0.0) || !(seconds <= 60.0)) return fail(nullptr, MR_ERR_INVALID_ARG, "mr_measure_fp64_peak: need 0 < seconds <= 60 and an output");
+    int dev = 0, sms = 0;
+    MR_CUDA(nullptr, cudaGetDevice(&dev));
+    MR_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int blocks = sms * 8, threads = 256;
+    const double flop_per_launch = 2.0 * kPeakChains * kPeakIters * (double)blocks * threads;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    MR_CUDA(nullptr, cudaEventCreate(&e0));
+    cudaError_t e = cudaEventCreate(&e1);
+    float ms = 0.f;
+    long long launches = 0;
+    if (e == cudaSuccess) {
+        // calibrate on three launches, then run as many as fill the time asked for between the two events
+        for (int q = 0; q < 3; ++q) k_fp64_chains<<<blocks, threads, 0, s>>>(1.0);
+        e = cudaEventRecord(e0, s);
+        k_fp64_chains<<<blocks, threads, 0, s>>>(1.0);
+        if (e == cudaSuccess) e = cudaEventRecord(e1, s);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e == cudaSuccess) {
+            launches = (long long)(seconds * 1e3 / (ms > 1e-3f ? ms : 1e-3f)) + 1;
+            e = cudaEventRecord(e0, s);
+            for (long long q = 0; q < launches; ++q) k_fp64_chains<<<blocks, threads, 0, s>>>(1.0);
+            if (e == cudaSuccess) e = cudaEventRecord(e1, s);
+            if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+            if (e == cudaSuccess) e = cudaGetLastError();
+        }
+    }
+    cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (e != cudaSuccess) return cuda_fail(nullptr, "mr_measure_fp64_peak", e);
+    *tflops = flop_per_launch * (double)launches / ((double)ms * 1e-3) / 1e12;
+    return MR_OK;
+}

@@ -107,6 +107,8 @@ lib.mr_set_variant.restype = C.c_int
 lib.mr_convexity_noalloc.argtypes = [C.c_void_p, C.POINTER(mr_grid), C.c_int, C.c_void_p, C.POINTER(C.c_int64), C.c_void_p]
 lib.mr_convexity_noalloc.restype = C.c_int
 NOALLOC_MAX_PLANES = 1024      # MR_NOALLOC_MAX_PLANES of include/mr.h
+lib.mr_measure_fp64_peak.argtypes = [C.c_double, C.c_void_p, C.POINTER(C.c_double)]
+lib.mr_measure_fp64_peak.restype = C.c_int
 
 
 class MrError(RuntimeError):
@@ -132,6 +134,18 @@ def workspace_bytes(n, dtype="f64", bc=("line_tied",) * 3) -> int:
 
 def _op(op):
     return OPERATORS[op] if isinstance(op, str) else int(op)
+
+
+def measure_fp64_peak(seconds, device=None):
+    """mr_measure_fp64_peak: TFLOP/s of a DFMA-chain kernel run for about ``seconds`` on the current stream of ``device``."""
+    import torch
+
+    out = C.c_double()
+    with torch.cuda.device(device):
+        st = lib.mr_measure_fp64_peak(float(seconds), torch.cuda.current_stream().cuda_stream, C.byref(out))
+    if st != MR_OK:
+        _raise(st, None)
+    return out.value
 
 
 def convexity_noalloc(x, kappa=None):

@@ -630,6 +630,15 @@ def test_context_on_a_side_stream_hands_its_results_to_the_callers_stream(mr):
             assert torch.equal(f[k], w[k]), (op, k)
 
 
+def test_fp64_peak_probe_is_plausible(mr):
+    """mr_measure_fp64_peak (the roofline denominator of bench.py --operator direct): a DFMA-chain kernel on a B200 delivers
+    between half and all of 148 SMs x 64 lanes x 2 FLOP x 1.965 GHz = 37.2 TFLOP/s."""
+    tf = mr.measure_fp64_peak(0.02)
+    assert 18.0 < tf < 38.0, tf
+    with pytest.raises(mr.MrError):
+        mr.measure_fp64_peak(0.0)
+
+
 def test_fp32_context_accepts_the_fp32_rounding_of_the_reference_grid(mr):
     """mr_set_x on an fp32 context: boundary nodes given as float32(X) are on the reference grid (|X|/h is large
     on config 5: 4 / (8/511)), one really displaced boundary node is still refused."""
