@@ -44,7 +44,7 @@ typedef enum {
     MR_ERR_INVALID_ARG = 1, /* null pointer, bad size, unsupported option */
     MR_ERR_WORKSPACE = 2,   /* workspace null, misaligned or too small */
     MR_ERR_CUDA = 3,        /* a CUDA runtime/driver call failed (no device, launch failure, ...) */
-    MR_ERR_STATE = 4,       /* B0 has not been set */
+    MR_ERR_STATE = 4,       /* B0 has not been set, a workspace is not bound, or mr_step_host_async calls are in flight */
     MR_ERR_NUMERIC = 5      /* det(dx/dX) <= 0 or a non-finite value was met (grid folded, cf. :333) */
 } mr_status;
 
